@@ -1,0 +1,331 @@
+"""Pins P0-P4, P7 of the CPU oracle (SURVEY.md 8(c) "What pins the oracle").
+
+Everything here is checked against something OTHER than the oracle itself:
+published Philox vectors, exact rational arithmetic, structural invariants of
+eq. (1) and the master equation built from the reaction list.
+CPU only (`-m "not gpu"`).
+"""
+import itertools
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ P0 ----
+def test_P0_philox_known_answers():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox_kat.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = oracle.philox4x32_10(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_P0_thresholds_exact_rational():
+    for line in open(os.path.join(GOLDEN, "thresholds.txt")):
+        if not line.strip() or line[0] == "#":
+            continue
+        q, T = line.split()
+        # exact: floor of (the IEEE double nearest q) * 2^32, in rationals
+        exact = (Fraction(float(q)) * (1 << 32)).__floor__()
+        assert oracle.threshold(float(q)) == exact == int(T, 16)
+    for bad in (-0.1, 1.0000001, float("nan")):
+        assert oracle.threshold(bad) == (1 << 64) - 1
+
+
+# ------------------------------------------------------------------ P0' ---
+def test_P0p_lane_uniforms_are_the_planes_transposed():
+    """U_j bit (31-k) = lane j of plane k; plane k = lo/hi of block k>>1 (C3),
+    rebuilt here from the KAT-pinned block function with numpy bit ops."""
+    seed, slot, sweep, word = 0x1234567890ABCDEF, 77, 5, 3
+    for stream in (oracle.STREAM_DIFF, oracle.STREAM_ANNI):
+        U = oracle.lane_uniforms(seed, slot, sweep, word, stream, 32)
+        planes = []
+        for m in range(16):
+            x = oracle.philox4x32_10([slot, sweep, word, (stream << 24) | m],
+                                     [seed & 0xFFFFFFFF, seed >> 32])
+            planes.append(int(x[0]) | (int(x[1]) << 32))
+            planes.append(int(x[2]) | (int(x[3]) << 32))
+        for j in range(64):
+            u = 0
+            for k in range(32):
+                u |= ((planes[k] >> j) & 1) << (31 - k)
+            assert u == int(U[j])
+
+
+def test_P0p_reduced_K_exhaustive_bitsliced_forms():
+    """For K = 4 every (U, T): direct compare == MSB-first (lt, und) form ==
+    LSB-first eager form (C3 'Equivalent bit-sliced forms').  The lanes come
+    from the oracle's reduced-K uniforms so that all 16 U values occur."""
+    K = 4
+    seen = set()
+    for slot in range(40):
+        U = oracle.lane_uniforms(9, slot, 0, 0, oracle.STREAM_DIFF, K)
+        seen |= set(int(u) for u in U)
+        planes = [sum((((int(U[j]) >> (K - 1 - k)) & 1) << j) for j in range(64)) for k in range(K)]
+        full = (1 << 64) - 1
+        for T in range(0, (1 << K) + 1):
+            direct = sum((1 << j) for j in range(64) if int(U[j]) < T)
+            if T == (1 << K):
+                assert direct == full
+                continue
+            lt, und = 0, full
+            for k in range(K):
+                bit = (T >> (K - 1 - k)) & 1
+                if bit:
+                    lt |= und & ~planes[k] & full
+                    und &= planes[k]
+                else:
+                    und &= ~planes[k] & full
+            assert lt == direct
+            m = 0
+            for k in reversed(range(K)):
+                bit = (T >> (K - 1 - k)) & 1
+                m = (m | (~planes[k] & full)) if bit else (m & ~planes[k] & full)
+            assert m == direct
+    assert seen == set(range(16))
+
+
+@pytest.mark.parametrize("q", [0.5, 0.15, 0.09, 0.8, 0.0, 1.0])
+def test_P0p_mask_frequency(q):
+    T = oracle.threshold(q)
+    n_masks = 4000  # 256k lanes
+    ones = 0
+    for slot in range(n_masks):
+        ones += int(oracle.bernoulli_mask(42, slot, 7, 1, oracle.STREAM_ANNI, T).sum())
+    n = 64 * n_masks
+    pr = T / 2.0 ** 32
+    sigma = (n * pr * (1 - pr)) ** 0.5
+    assert abs(ones - n * pr) <= 4 * sigma + 1e-9
+
+
+def test_P0p_streams_and_words_are_distinct():
+    a = oracle.lane_uniforms(1, 0, 0, 0, oracle.STREAM_DIFF)
+    assert not np.array_equal(a, oracle.lane_uniforms(1, 0, 0, 0, oracle.STREAM_ANNI))
+    assert not np.array_equal(a, oracle.lane_uniforms(1, 1, 0, 0, oracle.STREAM_DIFF))
+    assert not np.array_equal(a, oracle.lane_uniforms(1, 0, 1, 0, oracle.STREAM_DIFF))
+    assert not np.array_equal(a, oracle.lane_uniforms(1, 0, 0, 1, oracle.STREAM_DIFF))
+    assert not np.array_equal(a, oracle.lane_uniforms(2, 0, 0, 0, oracle.STREAM_DIFF))
+    assert not np.array_equal(a, oracle.lane_uniforms(1 << 32, 0, 0, 0, oracle.STREAM_DIFF))
+
+
+# ------------------------------------------------------------------ P1-P3 -
+SCHEDULES = [dict(Ts=2048, D=64, A=4), dict(Ts=64, D=64, A=64), dict(Ts=32, D=16, A=2)]
+
+
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("sch", SCHEDULES)
+def test_P1_empty_lattice_is_absorbing(variant, sch):
+    o = oracle.Oracle(128, 128, 0.3, 0.2, 11, variant, **sch)
+    o.init(wl.INIT_EMPTY)
+    o.run(5)
+    assert not o.get_words().any() and not o.counts().any()
+
+
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("sch", SCHEDULES)
+def test_P2_d_equals_one_conserves_particles(variant, sch):
+    o = oracle.Oracle(128, 128, 1.0, 0.3, 12, variant, **sch)
+    w0 = wl.random_lattice_words(128, 2, 0.4, seed=5)
+    o.set_words(w0)
+    c0 = o.counts()
+    for _ in range(4):
+        o.run(1)
+        assert np.array_equal(o.counts(), c0)
+    assert not np.array_equal(o.get_words(), w0)  # it did move
+
+
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+def test_P3_isolated_particles_never_react(variant):
+    # one particle per replica: count stays 1 for any d, p
+    L = 128
+    o = oracle.Oracle(L, 64, 0.4, 0.3, 13, variant, Ts=64, D=32, A=4)
+    w0 = np.zeros((L, 1), dtype=np.uint64)
+    rng = np.random.default_rng(0)
+    for j in range(64):
+        w0[rng.integers(0, L), 0] |= np.uint64(1) << np.uint64(j)
+    o.set_words(w0)
+    for _ in range(6):
+        o.run(1)
+        assert np.all(o.counts() == 1)
+    # d = 0: any state without adjacent pairs (triples) is frozen bit for bit
+    o = oracle.Oracle(L, 128, 0.0, 0.3, 14, variant, Ts=64, D=32, A=4)
+    w0 = wl.isolated_particles_words(L, 2, 4, seed=3)
+    o.set_words(w0)
+    o.run(4)
+    assert np.array_equal(o.get_words(), w0)
+
+
+def test_P3_tcpd_pairs_frozen_at_d0_but_pcpd_reacts():
+    L = 64
+    w0 = np.zeros((L, 1), dtype=np.uint64)
+    full = np.uint64(0xFFFFFFFFFFFFFFFF)
+    for i in range(0, L, 8):
+        w0[i, 0] = full
+        w0[i + 1, 0] = full  # isolated pairs, no triples
+    t = oracle.Oracle(L, 64, 0.0, 0.3, 15, wl.TCPD, Ts=64, D=16, A=4)
+    t.set_words(w0)
+    t.run(3)
+    assert np.array_equal(t.get_words(), w0)
+    p = oracle.Oracle(L, 64, 0.0, 0.3, 15, wl.PCPD, Ts=64, D=16, A=4)
+    p.set_words(w0)
+    p.run(3)
+    assert not np.array_equal(p.get_words(), w0)
+
+
+# ------------------------------------------------------------------ P4 ----
+def _bits(s, L):
+    return [(s >> i) & 1 for i in range(L)]
+
+
+def _state(bits):
+    return sum(b << i for i, b in enumerate(bits))
+
+
+def master_matrix(variant, L, d, p):
+    """One-attempt transition matrix P[s, s'] built from eq. (1)'s REACTION
+    LIST alone (TCPD: BASELINE.json config 5), exact rationals:
+    every bond/site i is selected with probability 1/L; hop at rate d if exactly
+    one end occupied; pair (triple) -> empty at p(1-d); creation at each EMPTY
+    outer neighbour at (1-p)(1-d)/2; diagonal by normalisation."""
+    n = 1 << L
+    P = [[Fraction(0)] * n for _ in range(n)]
+    k = 2 if variant == wl.PCPD else 3
+    for s in range(n):
+        b = _bits(s, L)
+        for i in range(L):
+            cluster = [(i + m) % L for m in range(k)]
+            lo, hi = (i - 1) % L, (i + k) % L
+            i1 = (i + 1) % L
+            if b[i] != b[i1]:
+                nb = list(b)
+                nb[i], nb[i1] = b[i1], b[i]
+                P[s][_state(nb)] += d / L
+            if all(b[c] for c in cluster):
+                nb = list(b)
+                for c in cluster:
+                    nb[c] = 0
+                P[s][_state(nb)] += p * (1 - d) / L
+                for tgt in (lo, hi):
+                    if not b[tgt]:
+                        nb = list(b)
+                        nb[tgt] = 1
+                        P[s][_state(nb)] += (1 - p) * (1 - d) / 2 / L
+        P[s][s] += 1 - sum(P[s])
+    return P
+
+
+def oracle_matrix(variant, L, d, p):
+    n = 1 << L
+    P = [[Fraction(0)] * n for _ in range(n)]
+    half = Fraction(1, 2)
+    for s in range(n):
+        b = _bits(s, L)
+        for i in range(L):
+            for Dm, Pm, Fm in itertools.product((0, 1), repeat=3):
+                wgt = (d if Dm else 1 - d) * (p if Pm else 1 - p) * half / L
+                out = oracle.single_attempt(variant, b, i, Dm, Pm, Fm)
+                P[s][_state([int(x) for x in out])] += wgt
+    return P
+
+
+@pytest.mark.parametrize("variant,L", [(wl.PCPD, 4), (wl.PCPD, 5), (wl.PCPD, 6), (wl.TCPD, 5), (wl.TCPD, 6)])
+def test_P4_master_equation_enumeration(variant, L):
+    d, p = Fraction(3, 10), Fraction(7, 40)
+    assert master_matrix(variant, L, d, p) == oracle_matrix(variant, L, d, p)  # exact rationals
+
+
+def test_P4_fission_side_follows_alg1():
+    # G8: Fm = 1 (r3 < 1/2) -> fission LOW (q_{i-1})
+    q = [0, 1, 1, 0, 0, 0]
+    assert list(oracle.single_attempt(wl.PCPD, q, 1, 0, 0, 1)) == [1, 1, 1, 0, 0, 0]
+    assert list(oracle.single_attempt(wl.PCPD, q, 1, 0, 0, 0)) == [0, 1, 1, 1, 0, 0]
+    # G3: diffusion has priority, a pair under Dm does not react
+    assert list(oracle.single_attempt(wl.PCPD, q, 1, 1, 1, 1)) == q
+    assert list(oracle.single_attempt(wl.PCPD, q, 1, 0, 1, 1)) == [0, 0, 0, 0, 0, 0]
+    assert list(oracle.single_attempt(wl.PCPD, q, 2, 1, 0, 0)) == [0, 1, 0, 1, 0, 0]
+    # periodic wrap (G2)
+    assert list(oracle.single_attempt(wl.PCPD, [1, 0, 0, 0, 0, 1], 5, 0, 0, 1)) == [1, 0, 0, 0, 1, 1]
+    assert list(oracle.single_attempt(wl.PCPD, [1, 0, 0, 0, 0, 1], 5, 0, 0, 0)) == [1, 1, 0, 0, 0, 1]
+
+
+@pytest.mark.parametrize("variant,L", [(wl.PCPD, 6), (wl.TCPD, 6)])
+def test_P4_literal_mode_mean_density_vs_master_equation(variant, L):
+    """E[count] after n = 1, 2, 3 time units (n*L attempts) from P^(nL) (floats
+    from the exact-rational matrix) vs the literal Alg. 1 Monte Carlo mean."""
+    d, p = 0.3, 0.175
+    P = np.array([[float(x) for x in row] for row in
+                  master_matrix(variant, L, Fraction(3, 10), Fraction(7, 40))])
+    pop = np.array([bin(s).count("1") for s in range(1 << L)], dtype=float)
+    R = 200_000
+    q0 = np.ones((R, L), dtype=np.uint8)
+    counts, _ = oracle.literal_run(variant, L, R, d, p, 99, q0, [0, 1, 2, 3])
+    v = np.zeros(1 << L)
+    v[(1 << L) - 1] = 1.0
+    for n in range(4):
+        exact_mean = v @ pop
+        exact_var = v @ pop ** 2 - exact_mean ** 2
+        mc = counts[n].mean()
+        assert abs(mc - exact_mean) <= 4.5 * (exact_var / R) ** 0.5 + 1e-12, (n, mc, exact_mean)
+        v = v @ np.linalg.matrix_power(P, L)
+
+
+# ------------------------------------------------------------------ P7 ----
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+def test_P7_run_splitting_loop_order_word_subsets(variant):
+    kw = dict(L=256, n_replicas=256, d=0.3, p=0.12, seed=21, variant=variant, Ts=128, D=32, A=4)
+    a = oracle.Oracle(**kw)
+    a.init(wl.INIT_BERNOULLI)
+    a.run(5)
+    b = oracle.Oracle(**kw)
+    b.init(wl.INIT_BERNOULLI)
+    b.run(2)
+    b.run(3)
+    assert np.array_equal(a.get_words(), b.get_words()) and a.sweep == b.sweep == 5
+    c = oracle.Oracle(**kw)
+    c.set_reverse_order(1)
+    c.init(wl.INIT_BERNOULLI)
+    c.run(5)
+    assert np.array_equal(a.get_words(), c.get_words())
+    s = oracle.Oracle(**kw, words=[3, 1])
+    s.init(wl.INIT_BERNOULLI)
+    s.run(5)
+    assert np.array_equal(a.get_words()[:, [3, 1]], s.get_words())
+    assert np.array_equal(a.counts().reshape(4, 64)[[3, 1]].ravel(), s.counts())
+    # set/get round trip and counts = column popcounts
+    w = a.get_words()
+    bits = (w[:, :, None] >> np.arange(64, dtype=np.uint64)) & np.uint64(1)
+    assert np.array_equal(bits.sum(axis=0).ravel().astype(np.uint32), a.counts())
+    s2 = oracle.Oracle(**kw)
+    s2.set_words(w)
+    assert np.array_equal(s2.get_words(), w)
+
+
+def test_init_bernoulli_is_the_init_stream():
+    """C8: word(i, w) = lo of block (i, 0, w, 4<<24)."""
+    o = oracle.Oracle(64, 128, 0.5, 0.1, 0xABCDEF0123, 0, Ts=64, D=16, A=4)
+    o.init(wl.INIT_BERNOULLI)
+    w = o.get_words()
+    for i, k in [(0, 0), (5, 1), (63, 0)]:
+        x = oracle.philox4x32_10([i, 0, k, 4 << 24], [0xCDEF0123, 0xAB])
+        assert int(w[i, k]) == int(x[0]) | (int(x[1]) << 32)
+    frac = np.unpackbits(w.view(np.uint8)).mean()
+    assert abs(frac - 0.5) < 4 * 0.5 / (64 * 128) ** 0.5
+
+
+def test_create_rejects_invalid():
+    for kw in (dict(L=100, Ts=64, D=16, A=4), dict(L=128, Ts=64, D=24, A=4),
+               dict(L=128, Ts=64, D=16, A=3), dict(L=128, Ts=6, D=6, A=2)):
+        with pytest.raises(ValueError):
+            oracle.Oracle(kw["L"], 64, 0.5, 0.1, 1, 0, Ts=kw["Ts"], D=kw["D"], A=kw["A"])
+    with pytest.raises(ValueError):
+        oracle.Oracle(128, 64, 1.5, 0.1, 1, 0)
+    with pytest.raises(ValueError):
+        oracle.Oracle(128, 64, 0.5, 0.1, 1, 0, Ts=8, D=8, A=2).__class__(128, 64, 0.5, 0.1, 1, 1, Ts=8, D=8, A=2)  # TCPD needs D>=9

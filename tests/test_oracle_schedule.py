@@ -1,0 +1,185 @@
+"""Pins P5 and P6 of the oracle's schedule SD2.
+
+P6: exact operator calculation on a toy ring, written here from the text of C5
+and eq. (1) with numpy (shares nothing with the oracle except the KAT-pinned
+Philox block used to derive the shifts), compared with the oracle's Monte Carlo
+occupation and pair probabilities, site by site.
+P5: SD2 vs the literal Algorithm 1, mean density at log-spaced
+times - the paper's own way of validating a modified site selection
+(PAPER.md:191-197).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+
+# ------------------------------------------------------------------ P6 ----
+def rule_matrix(variant, nsites, x, d, p):
+    """Stochastic matrix M[s', s] of ONE attempt at domain-local pair position
+    x on `nsites` sites, from eq. (1)'s reaction list."""
+    k = 2 if variant == wl.PCPD else 3
+    n = 1 << nsites
+    M = np.zeros((n, n))
+    for s in range(n):
+        b = [(s >> i) & 1 for i in range(nsites)]
+        stay = 1.0
+        if b[x] != b[x + 1]:
+            nb = list(b)
+            nb[x], nb[x + 1] = b[x + 1], b[x]
+            M[sum(v << i for i, v in enumerate(nb)), s] += d
+            stay -= d
+        if all(b[x + m] for m in range(k)):
+            nb = list(b)
+            for m in range(k):
+                nb[x + m] = 0
+            M[sum(v << i for i, v in enumerate(nb)), s] += p * (1 - d)
+            stay -= p * (1 - d)
+            for tgt in (x - 1, x + k):
+                if not b[tgt]:
+                    nb = list(b)
+                    nb[tgt] = 1
+                    M[sum(v << i for i, v in enumerate(nb)), s] += (1 - p) * (1 - d) / 2
+                    stay -= (1 - p) * (1 - d) / 2
+        M[s, s] += stay
+    return M
+
+
+def allowed_positions(D, Rr, c):
+    """C5 step 4: x in [1, D-1-Rr] minus (seam at c) x in [c-Rr, c]."""
+    xs = list(range(1, D - 1 - Rr + 1))
+    if c is not None:
+        xs = [x for x in xs if not (c - Rr <= x <= c)]
+    return xs
+
+
+def apply_on_sites(v, M, sites, L):
+    t = v.reshape((2,) * L)
+    # numpy axis a <-> site (L-1-a) when the state index has bit i = site i
+    axes = [L - 1 - s for s in sites]
+    t = np.moveaxis(t, axes[::-1], range(len(sites)))  # leading index bits: site[-1] is MSB
+    shp = t.shape
+    t = (M @ t.reshape(1 << len(sites), -1)).reshape(shp)
+    t = np.moveaxis(t, range(len(sites)), axes[::-1])
+    return np.ascontiguousarray(t).reshape(-1)
+
+
+def shifts_from_contract(seed, t, S, D, Ts):
+    """C5 step 1 from the KAT-pinned block function."""
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    sig = []
+    Sigma = None
+    for k in range(S):
+        x = oracle.philox4x32_10([k, t, 0, 3 << 24], key)
+        sig.append((int(x[0]) * D) >> 32)
+        if k == 0:
+            Sigma = (int(x[1]) * Ts) >> 32
+    return Sigma, sig
+
+
+@pytest.mark.parametrize("variant,L,Ts,D,A,sweeps", [
+    (wl.PCPD, 16, 16, 8, 2, 3),
+    (wl.PCPD, 16, 8, 8, 8, 3),
+    (wl.PCPD, 14, 14, 7, 1, 2),
+    (wl.TCPD, 18, 18, 9, 3, 3),
+])
+def test_P6_exact_schedule_operator_on_toy_ring(variant, L, Ts, D, A, sweeps):
+    d, p, seed = 0.3, 0.2, 1234
+    Rr = 2 if variant == wl.PCPD else 3
+    n, S, ntiles = Ts // D, D // A, L // Ts
+    R = 64 * 12000
+    o = oracle.Oracle(L, R, d, p, seed, variant, Ts=Ts, D=D, A=A)
+    o.init(wl.INIT_FULL)
+
+    mats = {x: rule_matrix(variant, D, x, d, p) for x in range(1, D - 1 - Rr + 1)}
+
+    def domain_op(c):
+        xs = allowed_positions(D, Rr, c)
+        one = sum(mats[x] for x in xs) / len(xs)
+        return np.linalg.matrix_power(one, A)
+
+    v = np.zeros(1 << L)
+    v[(1 << L) - 1] = 1.0
+    site_bit = np.array([[(s >> i) & 1 for i in range(L)] for s in range(1 << L)], dtype=float)
+    pair_bit = site_bit * np.roll(site_bit, -1, axis=1)
+    for t in range(sweeps):
+        Sigma, sig = shifts_from_contract(seed, t, S, D, Ts)
+        oS, osig = o.shifts(t, S)
+        assert oS == Sigma and list(osig) == sig
+        for k in range(S):
+            for tau in range(ntiles):
+                for b in range(n):
+                    seam = (D - sig[k]) if (b == n - 1 and sig[k] > 0) else None
+                    sites = [(Sigma + tau * Ts + (sig[k] + b * D + x) % Ts) % L for x in range(D)]
+                    v = apply_on_sites(v, domain_op(seam), sites, L)
+        o.run(1)
+        assert abs(v.sum() - 1) < 1e-12
+        words = o.get_words()  # [L, W]
+        bits = ((words[:, :, None] >> np.arange(64, dtype=np.uint64)) & np.uint64(1)).astype(np.float64)
+        # words (not replicas) are the independent samples (reading G12)
+        occ_w = bits.mean(axis=2)                                  # [L, W]
+        pair_w = (bits * np.roll(bits, -1, axis=0)).mean(axis=2)   # [L, W]
+        W = occ_w.shape[1]
+        for exact, samp in ((v @ site_bit, occ_w), (v @ pair_bit, pair_w)):
+            mean = samp.mean(axis=1)
+            err = samp.std(axis=1, ddof=1) / W ** 0.5
+            z = (mean - exact) / np.maximum(err, 1e-9)
+            assert np.all(np.abs(z) < 4.5), (t, z)
+
+
+def test_P6_shift_distribution_uniform():
+    """sigma_k uniform on [0, D), Sigma uniform on [0, Ts) (mulhi32 of the SHIFT
+    block), chi-square over many sweeps."""
+    D, Ts, A = 16, 64, 4
+    o = oracle.Oracle(128, 64, 0.5, 0.1, 5, 0, Ts=Ts, D=D, A=A)
+    cs, cS = np.zeros(D), np.zeros(Ts)
+    N = 6000
+    for t in range(N):
+        Sg, sg = o.shifts(t, D // A)
+        cS[Sg] += 1
+        for s in sg:
+            cs[s] += 1
+    chi_s = ((cs - cs.mean()) ** 2 / cs.mean()).sum()
+    chi_S = ((cS - cS.mean()) ** 2 / cS.mean()).sum()
+    assert chi_s < (D - 1) + 5 * (2 * (D - 1)) ** 0.5
+    assert chi_S < (Ts - 1) + 5 * (2 * (Ts - 1)) ** 0.5
+
+
+# ------------------------------------------------------------------ P5 ----
+def _sd2_vs_literal(variant, L, R, d, p, times, sch, seed=7):
+    W = R // 64
+    o = oracle.Oracle(L, R, d, p, seed, variant, **sch)
+    o.init(wl.INIT_FULL)
+    sd2 = []
+    prev = 0
+    for t in times:
+        o.run(t - prev)
+        prev = t
+        sd2.append(o.counts().astype(np.float64).reshape(W, 64).mean(axis=1) / L)  # per word
+    sd2 = np.array(sd2)                                                       # [n_t, W]
+    lit, _ = oracle.literal_run(variant, L, R, d, p, seed + 1000, np.ones((R, L), np.uint8), times)
+    lit = lit.astype(np.float64) / L                                          # [n_t, R]
+    m_s, e_s = sd2.mean(axis=1), sd2.std(axis=1, ddof=1) / W ** 0.5
+    m_l, e_l = lit.mean(axis=1), lit.std(axis=1, ddof=1) / R ** 0.5
+    z = (m_s - m_l) / np.sqrt(e_s ** 2 + e_l ** 2)
+    rel = m_s / m_l - 1
+    return z, rel, m_s, m_l
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("d,p", [(0.5, 0.15), (0.1, 0.09)])
+def test_P5_sd2_matches_literal_alg1(d, p):
+    times = [1, 2, 4, 8, 16, 32, 64]
+    z, rel, m_s, m_l = _sd2_vs_literal(wl.PCPD, 512, 2048, d, p, times, dict(Ts=2048, D=64, A=4))
+    print("P5", d, p, "z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)
+    assert np.all(np.abs(rel) < 0.02), rel
+
+
+@pytest.mark.slow
+def test_P5_tcpd_sd2_matches_literal():
+    times = [1, 2, 4, 8, 16, 32]
+    z, rel, _, _ = _sd2_vs_literal(wl.TCPD, 512, 1024, 0.5, 0.05, times, dict(Ts=2048, D=64, A=4))
+    print("P5 tcpd z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)
