@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py - replica-site updates/s of the PCPD multispin hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl ours|reference]
+
+One STEP = one pass of the hot path over one batch of synthetic input:
+`pcpd_run(SWEEPS_PER_STEP)` (RNG + masks + schedule + bitwise rule, SURVEY.md
+8(a) a1-a3) followed by `pcpd_density` (a4).  Init (a5) runs once before the
+warm-up and is timed separately (config.init_ms).  Workload at N = 1:
+BASELINE.json configs[3] ("cfg4": L = 2^22, 2048 replicas, 1 GiB lattice,
+d = 0.8, p = 0.12, full start, seed 4), the configuration the metric is quoted
+on.  N > 1: every rank runs its own cfg4-sized shard of word columns
+(word_offset = rank * W; no data-path collective) - weak scaling.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 7 for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import workloads as wl
+
+SWEEPS_PER_STEP = 10
+METRIC = "replica_site_updates_per_sec"
+UNIT = "replica-site updates/s"
+
+
+# --------------------------------------------------------------------------
+# Algorithmic instruction count per attempt-word (SURVEY.md
+# 8(d)): fixed part F + per-Philox-block cost * lazily-needed blocks, where the
+# number of blocks needed to decide all 64 lanes of a generic mask is
+# sum_m [1 - (1 - 4^-m)^64] (a lane stays undecided after k planes w.p. 2^-k).
+def blocks_needed_generic(nplanes: int) -> float:
+    nblk_max = (nplanes + 1) // 2
+    return sum(1.0 - (1.0 - 4.0 ** (-m)) ** 64 for m in range(nblk_max))
+
+
+def nplanes_of(q: float) -> int:
+    T = int(math.floor(math.ldexp(q, 32)))
+    if T == 0 or T >= 1 << 32:
+        return 0
+    return 32 - ((T & -T).bit_length() - 1)
+
+
+INSTR_PER_BLOCK_LAZY = 51.0   # 20 IMAD.WIDE + 20 LOP3 + counter set-up + MSB-first compare of 2 planes
+INSTR_PER_BLOCK_EAGER = 46.0
+
+
+def algorithmic_instr_per_attempt_word(cfg: wl.Config) -> dict:
+    F = 90.0 if cfg.variant == wl.PCPD else 100.0
+    npd, npp = nplanes_of(cfg.d), nplanes_of(cfg.p)
+    lazy_blocks = blocks_needed_generic(npd) + blocks_needed_generic(npp)
+    eager_blocks = (npd + 1) // 2 + (npp + 1) // 2
+    return dict(lazy=F + INSTR_PER_BLOCK_LAZY * lazy_blocks, eager=F + INSTR_PER_BLOCK_EAGER * eager_blocks,
+                lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=F)
+
+
+def load_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# --------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clocks and throttle reasons DURING the timed region (NVML)."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+
+    def start(self):
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+            return
+        self._thr = threading.Thread(target=self._loop, daemon=True)
+        self._thr.start()
+
+    def _loop(self):
+        nv = self._nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr:
+            self._thr.join(timeout=2)
+        s = sorted(self.samples)
+        return dict(sm_mhz=(s[len(s) // 2] if s else None), sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons),
+                    samples=len(s))
+
+
+# --------------------------------------------------------------------------
+def oracle_sample_rate(cfg: wl.Config, L_sample: int, n_cols: int, sweeps: int = 1) -> tuple[float, float]:
+    """Times the CPU oracle AS IT STANDS on `n_cols` word columns (one thread
+    each; ctypes releases the GIL) of a ring of L_sample sites with the config's
+    d, p, variant, seed and schedule.  Returns (updates/s, seconds)."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+
+    handles = []
+    for w in range(n_cols):
+        o = oracle.Oracle(L_sample, cfg.n_replicas, cfg.d, cfg.p, cfg.seed, cfg.variant, words=[w])
+        o.init(cfg.init)
+        handles.append(o)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(n_cols) as ex:
+        list(ex.map(lambda o: o.run(sweeps), handles))
+    dt = time.perf_counter() - t0
+    for o in handles:
+        o.close()
+    return L_sample * 64.0 * n_cols * sweeps / dt, dt
+
+
+def reference_arm(args, cfg: wl.Config) -> None:
+    """--impl reference: there is no reference implementation (paper only), so
+    this arm times the ORACLE on the box's host cores on the same config,
+    metric and unit; each step = one sweep of a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = max(1, min(os.cpu_count() or 1, cfg.W, 16))
+    L_sample = min(cfg.L, 1 << 15)
+    for _ in range(args.warmup):
+        oracle_sample_rate(cfg, L_sample, cores, 1)
+    t_total, units = 0.0, 0.0
+    for _ in range(args.steps):
+        rate, dt = oracle_sample_rate(cfg, L_sample, cores, 1)
+        t_total += dt
+        units += rate * dt
+    value = units / t_total
+    sample = (f"{cfg.name} parameters (d, p, variant, seed, schedule) on a ring of L = {L_sample} sites, "
+              f"word columns 0..{cores - 1} of {cfg.W}, one sweep per step, one thread per column")
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * t_total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="u8", data="synthetic", impl="reference",
+                config=dict(workload=cfg.name, L=cfg.L, n_replicas=cfg.n_replicas, d=cfg.d, p=cfg.p,
+                            variant="PCPD" if cfg.variant == wl.PCPD else "TCPD", sample=sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+def ours_arm(args, cfg: wl.Config) -> None:
+    import torch
+    import torch.distributed as dist
+
+    import paper_1301_6082_b200 as pk
+    from paper_1301_6082_b200 import build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the PCPD path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    peaks = load_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # weak scaling: every rank owns a cfg-sized shard of word columns of an N x bigger run
+    h = pk.Pcpd(cfg.L, cfg.n_replicas, cfg.d, cfg.p, cfg.seed, cfg.variant, word_offset=rank * cfg.W)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record()
+    h.init(cfg.init)
+    ev[1].record()
+    torch.cuda.synchronize()
+    init_ms = ev[0].elapsed_time(ev[1])
+    counts = np.empty(cfg.n_replicas, dtype=np.uint32)
+
+    def step():
+        h.run(SWEEPS_PER_STEP)
+        h.density(counts)
+
+    for _ in range(args.warmup):
+        step()
+
+    # ---- timed region 1: device-resident (value) ---------------------------
+    sampler = ClockSampler(local_rank)
+    barrier()
+    l0 = pk.launch_count()
+    sampler.start()
+    ev[0].record()
+    for _ in range(args.steps):
+        step()
+    ev[1].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = pk.launch_count() - l0
+    t_ms = torch.tensor([ev[0].elapsed_time(ev[1])], device="cuda")
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    t_ms = float(t_ms.item())
+    units_per_step = float(cfg.L) * cfg.n_replicas * SWEEPS_PER_STEP * world
+    value = units_per_step * args.steps / (t_ms * 1e-3)
+
+    # ---- dominant kernel alone: sweep kernel launch durations ---------------
+    n_k = max(4, min(40, args.steps * SWEEPS_PER_STEP))
+    kev = [torch.cuda.Event(enable_timing=True) for _ in range(n_k + 1)]
+    torch.cuda.synchronize()
+    kev[0].record()
+    for i in range(n_k):
+        h.run(1)
+        kev[i + 1].record()
+    torch.cuda.synchronize()
+    sweep_ms = sum(kev[i].elapsed_time(kev[i + 1]) for i in range(n_k)) / n_k
+    # density kernel alone
+    ev[2].record()
+    for _ in range(3):
+        h.density(counts)
+    ev[3].record()
+    torch.cuda.synchronize()
+    density_ms = ev[2].elapsed_time(ev[3]) / 3
+
+    # ---- timed region 2: end to end through the C ABI with HOST buffers -----
+    host_lat = torch.empty((cfg.L, cfg.W), dtype=torch.int64).pin_memory()
+    host_cnt = torch.empty(cfg.n_replicas, dtype=torch.int32).pin_memory()
+    h.get_lattice_ptr(host_lat.data_ptr())
+    e2e_steps = max(2, min(args.steps, 5))
+
+    def e2e_step():
+        h.set_lattice_ptr(host_lat.data_ptr())       # H2D of the step's input lattice
+        h.run(SWEEPS_PER_STEP)
+        h.density_ptr(host_cnt.data_ptr())            # D2H of the step's result
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    ev[0].record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    ev[1].record()
+    barrier()
+    wall = time.perf_counter() - t0
+    e_ms = torch.tensor([max(ev[0].elapsed_time(ev[1]), 0.0)], device="cuda")
+    if world > 1:
+        dist.all_reduce(e_ms, op=dist.ReduceOp.MAX)
+    e2e_value = units_per_step * e2e_steps / (float(e_ms.item()) * 1e-3)
+
+    if rank == 0:
+        alg = algorithmic_instr_per_attempt_word(cfg)
+        attempt_words = float(cfg.L) * cfg.W                      # per sweep launch
+        issue_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6        # thread-instr/s, 4 schedulers x 32 lanes per SM
+        achieved = alg["lazy"] * attempt_words / (sweep_ms * 1e-3)
+        hbm_bytes = 2.0 * cfg.lattice_bytes
+        roof = dict(bound="alu", achieved=achieved / 1e12, peak=issue_peak / 1e12, unit="Tinstr/s",
+                    frac=achieved / issue_peak, traffic=None,
+                    kernel="sweep_kernel", launch_ms=sweep_ms,
+                    instr_per_attempt_word=alg["lazy"], lazy_blocks=alg["lazy_blocks"],
+                    frac_eager=alg["eager"] * attempt_words / (sweep_ms * 1e-3) / issue_peak,
+                    peak_source=f"148 SMs x 128 thread-instr/clk x {peaks['sm_max_mhz']:.0f} MHz (guide unit counts)",
+                    hbm=dict(achieved=hbm_bytes / (sweep_ms * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                             frac=hbm_bytes / (sweep_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], peak_source=peaks["source"]))
+        cores = max(1, min(os.cpu_count() or 1, cfg.W, 16))
+        L_sample = min(cfg.L, 1 << 17)
+        cpu_rate, cpu_dt = oracle_sample_rate(cfg, L_sample, cores, 1)
+        sample = (f"{cfg.name} parameters on a ring of L = {L_sample} sites, word columns 0..{cores - 1} of {cfg.W}, "
+                  f"1 sweep, one thread per column ({cpu_dt:.1f} s)")
+        line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=t_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="u64", data="synthetic",
+                    config=dict(workload=cfg.name, L=cfg.L, n_replicas=cfg.n_replicas, d=cfg.d, p=cfg.p,
+                                variant="PCPD" if cfg.variant == wl.PCPD else "TCPD", seed=cfg.seed,
+                                sweeps_per_step=SWEEPS_PER_STEP, step="pcpd_run(10) + pcpd_density",
+                                schedule=h.schedule_info(), lattice_bytes=cfg.lattice_bytes,
+                                l2="lattice (1 GiB at cfg4) is larger than L2; no flush needed" if cfg.lattice_bytes > 200e6
+                                else "lattice smaller than L2 (correctness config)",
+                                init_ms=init_ms, density_ms=density_ms, parallelism=f"replica-word shards x{world}"),
+                    roofline=roof,
+                    cpu_baseline=dict(value=cpu_rate, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                    e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=cfg.lattice_bytes,
+                             d2h_bytes_per_step=4 * cfg.n_replicas, steps=e2e_steps, wall_s=wall),
+                    gpu_launches=int(launches), clocks=clocks)
+        print(json.dumps(line), flush=True)
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg4", choices=sorted(wl.BY_NAME))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = wl.BY_NAME[args.config]
+    if args.impl == "reference":
+        reference_arm(args, cfg)
+    else:
+        ours_arm(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,143 @@
+/*
+ * pcpd.h - C ABI of libpcpd.so: the B200-native (sm_100a) hot path of
+ * arXiv 1301.6082 (Schram, "Reaction-diffusion model Monte Carlo simulations on
+ * the GPU"): multispin Monte Carlo update of the 1+1-D pair contact process
+ * with diffusion (PCPD, eq. (1); Alg. 1; bitwise
+ * form Alg. 2) and its TCPD variant, with 64
+ * independent replicas bit-packed per uint64 word (classic multispin coding,
+ * PAPER.md:94-96).
+ *
+ * Conventions
+ *   L sites, periodic.  R = n_replicas, W = R/64 words per site.  Word (i, w)
+ *   holds replicas 64w .. 64w+63 at site i; bit j <-> replica 64w+j.
+ *   CANONICAL order of a host lattice buffer: words[i*W + w].  (The device
+ *   layout is private: word-blocked [W/Wb][L][Wb].)
+ *   One sweep = one time unit = L attempted updates per replica.
+ *   The update schedule, random streams and mask definition are the contract
+ *   C1..C9 of DESIGN.md section 3 (SD2(T_s, D, A) shifted domains, Philox-4x32-10
+ *   keyed by seed / sweep / slot / word, K = 32-plane Bernoulli masks).
+ *
+ * All pointers are HOST pointers unless the name ends in _dev.  Buffers are
+ * caller-owned; the library owns all device memory of a handle.  Every call
+ * returns 0 (PCPD_OK) or a negative pcpd_status; pcpd_create* return NULL on
+ * error.  The message of the last error on the calling thread is available from
+ * pcpd_last_error().  No C++ exception crosses this boundary.  A handle is used
+ * by one host thread at a time; distinct handles are independent.  There is NO
+ * CPU fallback: without a CUDA device of compute capability 10.x every compute
+ * call fails with PCPD_ERR_DEVICE.
+ */
+#ifndef PCPD_H
+#define PCPD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define PCPD_API __attribute__((visibility("default")))
+#else
+#define PCPD_API
+#endif
+
+typedef struct pcpd_s pcpd_t;
+
+enum pcpd_status {
+    PCPD_OK = 0,
+    PCPD_ERR_ARG = -1,     /* invalid argument (see pcpd_last_error) */
+    PCPD_ERR_DEVICE = -2,  /* no usable sm_100 device / CUDA runtime error */
+    PCPD_ERR_ALLOC = -3,   /* device allocation failed */
+    PCPD_ERR_RANGE = -4    /* sweep counter would exceed 2^32 - 1 */
+};
+
+enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1 };
+enum pcpd_init_mode { PCPD_INIT_FULL = 0, PCPD_INIT_BERNOULLI = 1, PCPD_INIT_EMPTY = 2 };
+
+/* Default schedule constants of SD2 (C5). */
+#define PCPD_DEFAULT_TS 2048u
+#define PCPD_DEFAULT_D 64u
+#define PCPD_DEFAULT_A 4u
+
+/* ---- plumbing: device memory and stream come from the host framework ------
+ * Optional.  alloc(bytes, stream) returns a DEVICE pointer (NULL on failure),
+ * release(ptr) frees it.  The Python binding installs PyTorch's CUDA caching
+ * allocator here; without it the library uses cudaMalloc/cudaFree.  Process
+ * wide; call before pcpd_create. */
+typedef void *(*pcpd_alloc_fn)(size_t bytes, void *cuda_stream);
+typedef void (*pcpd_free_fn)(void *dev_ptr);
+PCPD_API int pcpd_set_allocator(pcpd_alloc_fn alloc, pcpd_free_fn release);
+
+/* cudaStream_t (as void*) every later call of this handle enqueues on.
+ * Default: the legacy default stream. */
+PCPD_API int pcpd_set_stream(pcpd_t *h, void *cuda_stream);
+
+/* ---- the path -------------------------------------------------------------
+ * pcpd_create: variant 0 = PCPD, 1 = TCPD.  Schedule SD2(2048, 64, 4).
+ * Errors (NULL): n_replicas == 0 or not a multiple of 64; L not a multiple of
+ * the domain length D, or L < D; T_s is clamped to L when L < T_s, otherwise
+ * L % T_s != 0 is an error; d, p outside [0,1] or NaN; L >= 2^32 or
+ * W >= 2^32; unknown variant; allocation failure; no sm_100 device. */
+PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant);
+
+/* Same with explicit schedule constants (D | T_s | L, A | D, D >= 2*Rr+3 with
+ * Rr = 2 PCPD / 3 TCPD; T_s*Wb*8 bytes must fit the 227 KB shared memory) and
+ * a global word offset: the handle simulates word columns
+ * word_offset .. word_offset + W - 1 of a larger run (multi-GPU sharding by
+ * replica words); columns never interact, so the union of
+ * shards is bit-identical to one big run. */
+PCPD_API pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant,
+                       uint32_t T_s, uint32_t D, uint32_t A, uint64_t word_offset);
+
+/* mode 0: all sites occupied; 1: i.i.d. Bernoulli(1/2) from the INIT stream
+ * (C8: word(i,w) = low 64 bits of block (i, 0, w, 4<<24)); 2: empty.
+ * Resets the sweep counter to 0.  Asynchronous. */
+PCPD_API int pcpd_init(pcpd_t *h, int mode);
+
+/* Advance sweeps t0 .. t0+n-1, t0 = the handle's counter, so that
+ * run(a); run(b) == run(a+b) bit for bit.  Asynchronous on the handle's stream.
+ * PCPD_ERR_RANGE if the counter would pass 2^32 - 1. */
+PCPD_API int pcpd_run(pcpd_t *h, uint64_t n_sweeps);
+
+/* out_counts[r] = number of particles of replica r (C9; density = count / L is
+ * the caller's division), r < n_replicas.  Synchronises the stream. */
+PCPD_API int pcpd_density(pcpd_t *h, uint32_t *out_counts);
+
+/* out_pairs[r] = number of adjacent occupied pairs sum_i q(i) q(i+1) of
+ * replica r (pair density of PAPER.md:203-208, Figs 5-6).  Synchronises. */
+PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
+
+/* Lattice in canonical order words[i*W + w], L*W uint64.  Synchronise. */
+PCPD_API int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words);
+PCPD_API int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words);
+
+/* Schedule / precision constants in force for this handle (T_s after
+ * clamping; K = 32 planes), so an independent implementation can be run with
+ * the same ones.  Any out pointer may be NULL. */
+PCPD_API int pcpd_schedule_info(const pcpd_t *h, uint32_t *T_s, uint32_t *D, uint32_t *A, uint32_t *K);
+
+/* 32-bit-resolution thresholds T_d, T_p = floor(q * 2^32) in force (C3). */
+PCPD_API int pcpd_thresholds(const pcpd_t *h, uint64_t *T_d, uint64_t *T_p);
+
+PCPD_API uint64_t pcpd_sweep(const pcpd_t *h);           /* current sweep counter      */
+PCPD_API int pcpd_set_sweep(pcpd_t *h, uint64_t sweep);  /* checkpoint/resume          */
+PCPD_API int pcpd_synchronize(pcpd_t *h);                /* cudaStreamSynchronize      */
+PCPD_API void pcpd_destroy(pcpd_t *h);                   /* NULL-safe                  */
+PCPD_API const char *pcpd_last_error(void);              /* thread-local, library-owned */
+
+/* Number of kernels this library has launched so far in this process. */
+PCPD_API uint64_t pcpd_launch_count(void);
+
+/* ---- roofline microbenchmarks -----------------------
+ * Runs `iters` dependent-chain iterations of one instruction mix on every SM
+ * and returns the achieved rate in out_rate (thread-instructions per second,
+ * or Philox blocks per second for kind 3), timed with CUDA events.
+ * kind 0: LOP3 only; 1: IMAD.WIDE.U32 + LOP3 pairs (a Philox round's mix; rate
+ * counts both); 2: 32-bit IMAD only; 3: Philox-4x32-10 blocks. */
+PCPD_API int pcpd_microbench(int kind, uint32_t iters, double *out_rate);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCPD_H */

@@ -1,0 +1,236 @@
+"""paper_1301_6082_b200 - thin Python binding of libpcpd.so (include/pcpd.h).
+
+Argument marshalling only: every step of the path (RNG, masks, schedule, update
+rule, density reduction) runs in the CUDA kernels of csrc/.  PyTorch is used for
+device memory (its CUDA caching allocator is installed as the library's
+allocator) and for the stream (torch's current stream), nothing else.  There is
+no CPU fallback: if libpcpd.so is missing or no B200 is present, calls raise.
+
+Names follow the C ABI: pcpd_create / pcpd_init / pcpd_run / pcpd_density ...
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .shard import gather_counts, max_over_ranks, shard_words  # noqa: F401
+
+PCPD, TCPD = 0, 1
+INIT_FULL, INIT_BERNOULLI, INIT_EMPTY = 0, 1, 2
+DEFAULT_TS, DEFAULT_D, DEFAULT_A = 2048, 64, 4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpcpd.so")
+
+# every symbol include/pcpd.h declares
+EXPORTS = (
+    "pcpd_set_allocator", "pcpd_set_stream", "pcpd_create", "pcpd_create_ex", "pcpd_init", "pcpd_run",
+    "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
+    "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
+    "pcpd_launch_count", "pcpd_microbench",
+)
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p)
+
+_lib = None
+_keepalive = []
+
+
+class PcpdError(RuntimeError):
+    pass
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree libpcpd.so and declare the signatures.  Fails loudly
+    when the extension has not been built (python -m paper_1301_6082_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise PcpdError(f"{LIB_PATH} is missing: run `python -m paper_1301_6082_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(LIB_PATH)
+    u32p, u64p = C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
+    L.pcpd_set_allocator.argtypes = [_ALLOC_FN, _FREE_FN]
+    L.pcpd_set_allocator.restype = C.c_int
+    L.pcpd_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    L.pcpd_set_stream.restype = C.c_int
+    L.pcpd_create.argtypes = [C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_uint64, C.c_int]
+    L.pcpd_create.restype = C.c_void_p
+    L.pcpd_create_ex.argtypes = [C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_uint64, C.c_int,
+                                 C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64]
+    L.pcpd_create_ex.restype = C.c_void_p
+    L.pcpd_init.argtypes = [C.c_void_p, C.c_int]
+    L.pcpd_init.restype = C.c_int
+    L.pcpd_run.argtypes = [C.c_void_p, C.c_uint64]
+    L.pcpd_run.restype = C.c_int
+    L.pcpd_density.argtypes = [C.c_void_p, C.c_void_p]
+    L.pcpd_density.restype = C.c_int
+    L.pcpd_pair_density.argtypes = [C.c_void_p, C.c_void_p]
+    L.pcpd_pair_density.restype = C.c_int
+    L.pcpd_get_lattice.argtypes = [C.c_void_p, C.c_void_p]
+    L.pcpd_get_lattice.restype = C.c_int
+    L.pcpd_set_lattice.argtypes = [C.c_void_p, C.c_void_p]
+    L.pcpd_set_lattice.restype = C.c_int
+    L.pcpd_schedule_info.argtypes = [C.c_void_p, u32p, u32p, u32p, u32p]
+    L.pcpd_schedule_info.restype = C.c_int
+    L.pcpd_thresholds.argtypes = [C.c_void_p, u64p, u64p]
+    L.pcpd_thresholds.restype = C.c_int
+    L.pcpd_sweep.argtypes = [C.c_void_p]
+    L.pcpd_sweep.restype = C.c_uint64
+    L.pcpd_set_sweep.argtypes = [C.c_void_p, C.c_uint64]
+    L.pcpd_set_sweep.restype = C.c_int
+    L.pcpd_synchronize.argtypes = [C.c_void_p]
+    L.pcpd_synchronize.restype = C.c_int
+    L.pcpd_destroy.argtypes = [C.c_void_p]
+    L.pcpd_destroy.restype = None
+    L.pcpd_last_error.argtypes = []
+    L.pcpd_last_error.restype = C.c_char_p
+    L.pcpd_launch_count.argtypes = []
+    L.pcpd_launch_count.restype = C.c_uint64
+    L.pcpd_microbench.argtypes = [C.c_int, C.c_uint32, C.POINTER(C.c_double)]
+    L.pcpd_microbench.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _install_torch_allocator(L: C.CDLL) -> None:
+    """PyTorch for device memory: route the library's allocations through
+    torch's CUDA caching allocator."""
+    if _keepalive:
+        return
+    import torch
+
+    def _alloc(nbytes, stream):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+        except Exception:
+            return None
+
+    def _free(ptr):
+        torch.cuda.caching_allocator_delete(ptr)
+
+    a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
+    _keepalive.extend([a, f])
+    L.pcpd_set_allocator(a, f)
+
+
+def _err(L) -> str:
+    return (L.pcpd_last_error() or b"").decode()
+
+
+def _check(L, rc):
+    if rc != 0:
+        raise PcpdError(f"libpcpd error {rc}: {_err(L)}")
+
+
+def launch_count() -> int:
+    return int(load_library().pcpd_launch_count())
+
+
+def microbench(kind: int, iters: int = 2000) -> float:
+    L = load_library()
+    out = C.c_double()
+    _check(L, L.pcpd_microbench(kind, iters, C.byref(out)))
+    return out.value
+
+
+class Pcpd:
+    """One simulation handle (pcpd_t).  Methods mirror the C ABI one to one."""
+
+    def __init__(self, L, n_replicas, d, p, seed, variant=PCPD, Ts=None, D=None, A=None, word_offset=0):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise PcpdError("no CUDA device: the PCPD path has no CPU fallback")
+        lib = load_library()
+        _install_torch_allocator(lib)
+        self._lib = lib
+        torch.cuda.current_stream()  # make sure the context exists
+        if Ts is None and D is None and A is None and word_offset == 0:
+            h = lib.pcpd_create(L, n_replicas, d, p, seed, variant)
+        else:
+            h = lib.pcpd_create_ex(L, n_replicas, d, p, seed, variant, Ts or DEFAULT_TS, D or DEFAULT_D,
+                                   A or DEFAULT_A, word_offset)
+        if not h:
+            raise PcpdError(f"pcpd_create failed: {_err(lib)}")
+        self._h = h
+        self.L, self.n_replicas, self.W = int(L), int(n_replicas), int(n_replicas) // 64
+        self.use_current_stream()
+
+    # -- plumbing
+    def use_current_stream(self):
+        import torch
+
+        _check(self._lib, self._lib.pcpd_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.pcpd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the path
+    def init(self, mode=INIT_FULL):
+        _check(self._lib, self._lib.pcpd_init(self._h, mode))
+
+    def run(self, n_sweeps):
+        _check(self._lib, self._lib.pcpd_run(self._h, n_sweeps))
+
+    def density(self, out=None) -> np.ndarray:
+        out = np.empty(self.n_replicas, dtype=np.uint32) if out is None else out
+        _check(self._lib, self._lib.pcpd_density(self._h, out.ctypes.data))
+        return out
+
+    def pair_density(self, out=None) -> np.ndarray:
+        out = np.empty(self.n_replicas, dtype=np.uint32) if out is None else out
+        _check(self._lib, self._lib.pcpd_pair_density(self._h, out.ctypes.data))
+        return out
+
+    def get_lattice(self, out=None) -> np.ndarray:
+        out = np.empty((self.L, self.W), dtype=np.uint64) if out is None else out
+        _check(self._lib, self._lib.pcpd_get_lattice(self._h, out.ctypes.data))
+        return out
+
+    def set_lattice(self, words):
+        a = np.ascontiguousarray(words, dtype=np.uint64)
+        if a.size != self.L * self.W:
+            raise ValueError("lattice must hold L*W uint64 words in canonical order [i][w]")
+        _check(self._lib, self._lib.pcpd_set_lattice(self._h, a.ctypes.data))
+
+    def get_lattice_ptr(self, host_ptr: int):
+        _check(self._lib, self._lib.pcpd_get_lattice(self._h, host_ptr))
+
+    def set_lattice_ptr(self, host_ptr: int):
+        _check(self._lib, self._lib.pcpd_set_lattice(self._h, host_ptr))
+
+    def density_ptr(self, host_ptr: int):
+        _check(self._lib, self._lib.pcpd_density(self._h, host_ptr))
+
+    def schedule_info(self) -> dict:
+        v = [C.c_uint32() for _ in range(4)]
+        _check(self._lib, self._lib.pcpd_schedule_info(self._h, *[C.byref(x) for x in v]))
+        return dict(Ts=v[0].value, D=v[1].value, A=v[2].value, K=v[3].value)
+
+    def thresholds(self):
+        a, b = C.c_uint64(), C.c_uint64()
+        _check(self._lib, self._lib.pcpd_thresholds(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    @property
+    def sweep(self) -> int:
+        return int(self._lib.pcpd_sweep(self._h))
+
+    @sweep.setter
+    def sweep(self, t):
+        _check(self._lib, self._lib.pcpd_set_sweep(self._h, t))
+
+    def synchronize(self):
+        _check(self._lib, self._lib.pcpd_synchronize(self._h))

@@ -1,0 +1,361 @@
+// Host side of libpcpd.so: the C ABI declared in include/pcpd.h.
+// Argument checking, thresholds (C3), handle state (C7: lattice + sweep counter),
+// kernel launches.  No compute happens on the host; there is no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <atomic>
+#include <new>
+
+#include "../../include/pcpd.h"
+#include "pcpd_kernels.cuh"
+
+using namespace pcpd;
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<uint64_t> g_launches{0};
+pcpd_alloc_fn g_alloc = nullptr;
+pcpd_free_fn g_free = nullptr;
+bool g_configured = false;
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(PCPD_ERR_DEVICE, "%s: %s", what, cudaGetErrorString(e));
+}
+
+void *dev_alloc(size_t bytes, cudaStream_t s)
+{
+    if (g_alloc) return g_alloc(bytes, (void *)s);
+    void *p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    return p;
+}
+
+void dev_free(void *p)
+{
+    if (!p) return;
+    if (g_free) g_free(p);
+    else cudaFree(p);
+}
+
+// T = floor(q * 2^32) in double arithmetic (C3); q in [0,1].
+uint64_t threshold_of(double q) { return (uint64_t)std::floor(std::ldexp(q, 32)); }
+
+Threshold make_threshold(uint64_t T)
+{
+    Threshold th{};
+    th.all = (T >= (1ull << 32)) ? 1u : 0u;
+    th.T32 = th.all ? 0u : (uint32_t)T;
+    th.nplanes = (th.all || T == 0) ? 0u : 32u - (uint32_t)__builtin_ctz((uint32_t)T);
+    return th;
+}
+
+}  // namespace
+
+struct pcpd_s {
+    uint64_t L, R, W;
+    double d, p;
+    uint64_t seed;
+    int variant;
+    uint32_t Ts, D, A;
+    uint64_t word_offset;
+    uint64_t Td, Tp;
+    int Wb;
+    uint64_t sweep;
+    uint64_t *lat;     // device, word-blocked
+    uint32_t *counts;  // device, uint32[R]
+    cudaStream_t stream;
+    SweepParams P;
+};
+
+extern "C" {
+
+const char *pcpd_last_error(void) { return g_err; }
+uint64_t pcpd_launch_count(void) { return g_launches.load(); }
+
+int pcpd_set_allocator(pcpd_alloc_fn alloc, pcpd_free_fn release)
+{
+    if ((alloc == nullptr) != (release == nullptr)) return fail(PCPD_ERR_ARG, "set_allocator: give both or neither");
+    g_alloc = alloc;
+    g_free = release;
+    return PCPD_OK;
+}
+
+pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant, uint32_t Ts,
+                       uint32_t D, uint32_t A, uint64_t word_offset)
+{
+    if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD) {
+        fail(PCPD_ERR_ARG, "unknown variant %d", variant);
+        return nullptr;
+    }
+    const uint32_t Rr = variant == 0 ? 2u : 3u;
+    if (n_replicas == 0 || n_replicas % 64) {
+        fail(PCPD_ERR_ARG, "n_replicas must be a positive multiple of 64");
+        return nullptr;
+    }
+    const uint64_t W = n_replicas / 64;
+    if (!(d >= 0.0 && d <= 1.0) || !(p >= 0.0 && p <= 1.0)) {
+        fail(PCPD_ERR_ARG, "d and p must lie in [0,1]");
+        return nullptr;
+    }
+    if (L == 0 || L >= (1ull << 32) || word_offset + W >= (1ull << 32)) {
+        fail(PCPD_ERR_ARG, "L and word_offset + W must be < 2^32 (32-bit counter fields)");
+        return nullptr;
+    }
+    if (D == 0 || A == 0 || Ts == 0 || D % A) {
+        fail(PCPD_ERR_ARG, "schedule: need A | D, all non-zero");
+        return nullptr;
+    }
+    if (D < 2 * Rr + 3) {
+        fail(PCPD_ERR_ARG, "schedule: D must be >= %u for this variant", 2 * Rr + 3);
+        return nullptr;
+    }
+    if (L < D || L % D) {
+        fail(PCPD_ERR_ARG, "L must be a multiple of the domain length D = %u", D);
+        return nullptr;
+    }
+    if (Ts > L) Ts = (uint32_t)L;  // clamp
+    if (Ts % D || L % Ts) {
+        fail(PCPD_ERR_ARG, "schedule: need D | T_s | L (T_s = %u, D = %u)", Ts, D);
+        return nullptr;
+    }
+    if (D / A > MAX_SUBSTEPS) {
+        fail(PCPD_ERR_ARG, "schedule: D / A must be <= %u", MAX_SUBSTEPS);
+        return nullptr;
+    }
+    // word-group width: widest of 4, 2, 1 dividing W that fits shared memory / block size
+    int Wb = 1;
+    for (int cand = 4; cand >= 1; cand >>= 1) {
+        if (W % cand) continue;
+        if (sweep_smem_bytes(Ts, cand) > 200 * 1024) continue;
+        if ((uint64_t)(Ts / D) * cand > 1024) continue;
+        Wb = cand;
+        break;
+    }
+    if (sweep_smem_bytes(Ts, Wb) > 200 * 1024 || (uint64_t)(Ts / D) * Wb > 1024) {
+        fail(PCPD_ERR_ARG, "schedule: tile of %u sites does not fit one thread block", Ts);
+        return nullptr;
+    }
+    if (W / Wb > 65535) {
+        fail(PCPD_ERR_ARG, "too many word columns for one handle (W / %d > 65535): shard by word_offset", Wb);
+        return nullptr;
+    }
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) {
+        cuda_fail(e, "no CUDA device");
+        return nullptr;
+    }
+    if (prop.major != 10) {
+        fail(PCPD_ERR_DEVICE, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor);
+        return nullptr;
+    }
+    if (!g_configured) {
+        const int rc = configure_kernels();
+        if (rc != 0) {
+            cuda_fail((cudaError_t)rc, "cudaFuncSetAttribute");
+            return nullptr;
+        }
+        g_configured = true;
+    }
+
+    pcpd_s *h = new (std::nothrow) pcpd_s();
+    if (!h) {
+        fail(PCPD_ERR_ALLOC, "host allocation failed");
+        return nullptr;
+    }
+    h->L = L; h->R = n_replicas; h->W = W; h->d = d; h->p = p; h->seed = seed; h->variant = variant;
+    h->Ts = Ts; h->D = D; h->A = A; h->word_offset = word_offset; h->Wb = Wb; h->sweep = 0;
+    h->Td = threshold_of(d); h->Tp = threshold_of(p);
+    h->stream = nullptr;
+    h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
+    h->counts = (uint32_t *)dev_alloc(4 * n_replicas, h->stream);
+    if (!h->lat || !h->counts) {
+        dev_free(h->lat);
+        dev_free(h->counts);
+        delete h;
+        fail(PCPD_ERR_ALLOC, "device allocation of %llu bytes failed", (unsigned long long)(8 * L * W));
+        return nullptr;
+    }
+    SweepParams &P = h->P;
+    memset(&P, 0, sizeof P);
+    P.lat = h->lat; P.L = (uint32_t)L; P.W = (uint32_t)W; P.Ts = Ts; P.D = D; P.A = A; P.S = D / A; P.n = Ts / D;
+    P.word_offset = (uint32_t)word_offset;
+    P.thd = make_threshold(h->Td);
+    P.thp = make_threshold(h->Tp);
+    P.rk = make_round_keys(seed);
+    g_err[0] = 0;
+    return h;
+}
+
+pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant)
+{
+    return pcpd_create_ex(L, n_replicas, d, p, seed, variant, PCPD_DEFAULT_TS, PCPD_DEFAULT_D, PCPD_DEFAULT_A, 0);
+}
+
+void pcpd_destroy(pcpd_t *h)
+{
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    dev_free(h->lat);
+    dev_free(h->counts);
+    delete h;
+}
+
+int pcpd_set_stream(pcpd_t *h, void *cuda_stream)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    h->stream = (cudaStream_t)cuda_stream;
+    return PCPD_OK;
+}
+
+static int check_launch(const char *what)
+{
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    return PCPD_OK;
+}
+
+int pcpd_init(pcpd_t *h, int mode)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (mode < 0 || mode > 2) return fail(PCPD_ERR_ARG, "unknown init mode %d", mode);
+    g_launches += launch_init(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, (uint32_t)h->word_offset, mode, h->P.rk,
+                              h->stream);
+    h->sweep = 0;
+    return check_launch("init kernel");
+}
+
+int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    for (uint64_t it = 0; it < n_sweeps; ++it) {
+        h->P.t = (uint32_t)h->sweep;
+        g_launches += launch_sweep(h->P, h->variant, h->Wb, h->stream);
+        h->sweep += 1;
+    }
+    return check_launch("sweep kernel");
+}
+
+static int density_impl(pcpd_t *h, uint32_t *out, int pairs)
+{
+    if (!h || !out) return fail(PCPD_ERR_ARG, "null argument");
+    cudaError_t e = cudaMemsetAsync(h->counts, 0, 4 * h->R, h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset");
+    g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, pairs, h->counts, h->stream);
+    int rc = check_launch("density kernel");
+    if (rc) return rc;
+    e = cudaMemcpyAsync(out, h->counts, 4 * h->R, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "density read-back");
+    return PCPD_OK;
+}
+
+int pcpd_density(pcpd_t *h, uint32_t *out_counts) { return density_impl(h, out_counts, 0); }
+int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs) { return density_impl(h, out_pairs, 1); }
+
+int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words)
+{
+    if (!h || !out_words) return fail(PCPD_ERR_ARG, "null argument");
+    const size_t bytes = 8 * h->L * h->W;
+    cudaError_t e;
+    if ((uint64_t)h->Wb == h->W) {  // single word group: physical == canonical
+        e = cudaMemcpyAsync(out_words, h->lat, bytes, cudaMemcpyDeviceToHost, h->stream);
+    } else {
+        uint64_t *tmp = (uint64_t *)dev_alloc(bytes, h->stream);
+        if (!tmp) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
+        g_launches += launch_permute(h->lat, tmp, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 0, h->stream);
+        e = cudaMemcpyAsync(out_words, tmp, bytes, cudaMemcpyDeviceToHost, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        dev_free(tmp);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "get_lattice");
+    return check_launch("permute kernel");
+}
+
+int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words)
+{
+    if (!h || !in_words) return fail(PCPD_ERR_ARG, "null argument");
+    const size_t bytes = 8 * h->L * h->W;
+    cudaError_t e;
+    if ((uint64_t)h->Wb == h->W) {
+        e = cudaMemcpyAsync(h->lat, in_words, bytes, cudaMemcpyHostToDevice, h->stream);
+    } else {
+        uint64_t *tmp = (uint64_t *)dev_alloc(bytes, h->stream);
+        if (!tmp) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
+        e = cudaMemcpyAsync(tmp, in_words, bytes, cudaMemcpyHostToDevice, h->stream);
+        g_launches += launch_permute(tmp, h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 1, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        dev_free(tmp);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "set_lattice");
+    return check_launch("permute kernel");
+}
+
+int pcpd_schedule_info(const pcpd_t *h, uint32_t *Ts, uint32_t *D, uint32_t *A, uint32_t *K)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (Ts) *Ts = h->Ts;
+    if (D) *D = h->D;
+    if (A) *A = h->A;
+    if (K) *K = 32;
+    return PCPD_OK;
+}
+
+int pcpd_thresholds(const pcpd_t *h, uint64_t *Td, uint64_t *Tp)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (Td) *Td = h->Td;
+    if (Tp) *Tp = h->Tp;
+    return PCPD_OK;
+}
+
+uint64_t pcpd_sweep(const pcpd_t *h) { return h ? h->sweep : 0; }
+
+int pcpd_set_sweep(pcpd_t *h, uint64_t sweep)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (sweep > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter must be < 2^32");
+    h->sweep = sweep;
+    return PCPD_OK;
+}
+
+int pcpd_synchronize(pcpd_t *h)
+{
+    if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    const cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "synchronize");
+    return PCPD_OK;
+}
+
+int pcpd_microbench(int kind, uint32_t iters, double *out_rate)
+{
+    if (kind < 0 || kind > 3 || !out_rate || iters == 0) return fail(PCPD_ERR_ARG, "microbench: bad arguments");
+    const int rc = run_microbench(kind, iters, out_rate, nullptr);
+    g_launches += 4;
+    if (rc != 0) return fail(rc, "microbench failed");
+    return check_launch("microbench kernel");
+}
+
+}  // extern "C"

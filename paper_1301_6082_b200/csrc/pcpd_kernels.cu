@@ -1,0 +1,210 @@
+// Hand-written sm_100a kernels of the PCPD/TCPD multispin hot path
+// (DESIGN.md sections 4-5): sweep (RNG + masks + schedule + bitwise rule), init,
+// density (positional popcount), layout permutation.
+//
+// Citations: update rule = Alg. 1 PAPER.md:45-70 in the bitwise form of Alg. 2
+// PAPER.md:126-151 (typos fixed per DESIGN.md readings G5/G6); schedule SD2 and
+// streams = DESIGN.md section 3 C1-C9.
+#include "pcpd_kernels.cuh"
+
+namespace pcpd {
+
+__device__ __forceinline__ uint32_t mulhi32(uint32_t r, uint32_t n) { return __umulhi(r, n); }
+
+// ---------------------------------------------------------------------------
+// Bernoulli(T / 2^32) mask by MSB-first bit-sliced comparison of the 32 random
+// planes with the bits of T (C3), evaluated LAZILY: only lanes in `rel` (the
+// lanes on which the outcome can matter) are resolved, and the loop stops as
+// soon as every such lane is decided.  A lane is decided at the first plane
+// where its bit differs from T's bit; counter-based RNG makes the skipped
+// blocks free.  Returns lanes (within rel) with U < T.
+// Plane k (k even) = lo64, (k odd) = hi64 of block m = k >> 1 of `stream`.
+template <uint32_t STREAM>
+__device__ __forceinline__ uint64_t lazy_mask(uint64_t rel, const Threshold th, uint32_t slot, uint32_t t,
+                                              uint32_t w, const RoundKeys &rk)
+{
+    if (th.all) return rel;
+    uint64_t lt = 0, und = rel;
+    for (uint32_t k = 0; k < th.nplanes && und != 0; k += 2) {
+        const U4 blk = philox4x32_10(slot, t, w, STREAM | (k >> 1), rk);
+        // T's bit for plane k is bit (31 - k); thread-uniform.
+        const uint64_t tb0 = ((th.T32 >> (31 - k)) & 1u) ? ~0ull : 0ull;
+        const uint64_t tb1 = ((th.T32 >> (30 - k)) & 1u) ? ~0ull : 0ull;  // k <= 30
+        uint64_t pl = lo64(blk);
+        lt |= und & ~pl & tb0;   // T bit 1, lane bit 0 -> U < T
+        und &= ~(pl ^ tb0);      // stays undecided only where lane bit == T bit
+        pl = hi64(blk);
+        lt |= und & ~pl & tb1;
+        und &= ~(pl ^ tb1);
+    }
+    return lt;
+}
+
+// ---------------------------------------------------------------------------
+// One sweep of schedule SD2(Ts, D, A) (C5).  Grid (L/Ts tiles, W/WB word
+// groups); block = n * WB threads, thread (b, w') owns domain b of word column
+// w' for the whole sweep; the tile lives in shared memory from load to store,
+// so the lattice crosses HBM exactly once in each direction per sweep.
+template <int VARIANT, int WB>
+__global__ void sweep_kernel(const __grid_constant__ SweepParams P)
+{
+    extern __shared__ __align__(16) uint64_t tile[];  // [Ts][WB]
+    __shared__ uint32_t s_sigma[MAX_SUBSTEPS];
+    __shared__ uint32_t s_Sigma;
+
+    constexpr uint32_t Rr = VARIANT == 0 ? 2u : 3u;
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    const uint32_t tau = blockIdx.x, wg = blockIdx.y;
+    const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
+
+    // C5 step 1: shifts from the SHIFT stream.
+    for (uint32_t k = tid; k < S; k += nthr) {
+        const U4 blk = philox4x32_10(k, t, 0u, STREAM_SHIFT, P.rk);
+        s_sigma[k] = mulhi32(blk.x0, D);
+        if (k == 0) s_Sigma = mulhi32(blk.x1, Ts);
+    }
+    __syncthreads();
+
+    // C5 step 2: tile tau covers global sites (Sigma + tau*Ts + y) mod L.
+    const uint32_t start = (uint32_t)(((uint64_t)s_Sigma + (uint64_t)tau * Ts) % L);
+    uint64_t *g = P.lat + (size_t)wg * L * WB;
+    if constexpr (WB >= 2) {
+        constexpr uint32_t CPR = WB / 2;  // 16-byte chunks per site row
+        const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
+        ulonglong2 *t2 = reinterpret_cast<ulonglong2 *>(tile);
+        for (uint32_t c = tid; c < Ts * CPR; c += nthr) {
+            uint32_t i = start + c / CPR;
+            if (i >= L) i -= L;
+            t2[c] = g2[(size_t)i * CPR + c % CPR];
+        }
+    } else {
+        for (uint32_t y = tid; y < Ts; y += nthr) {
+            uint32_t i = start + y;
+            if (i >= L) i -= L;
+            tile[y] = g[i];
+        }
+    }
+    __syncthreads();
+
+    const uint32_t b = tid / WB, wl = tid % WB;
+    const uint32_t w = P.word_offset + wg * WB + wl;  // global word index (RNG key)
+    const uint32_t slot0 = (tau * n + b) * D;
+
+    for (uint32_t k = 0; k < S; ++k) {
+        const uint32_t sigma = s_sigma[k];
+        // C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
+        // domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
+        const bool seam = (b == n - 1) && (sigma > 0);
+        const int32_t c = (int32_t)D - (int32_t)sigma;
+        int32_t lo = 0, rem = 0;
+        if (seam) {
+            lo = max(1, c - (int32_t)Rr);
+            const int32_t hi = min((int32_t)D - 1 - (int32_t)Rr, c);
+            rem = max(0, hi - lo + 1);
+        }
+        const uint32_t n_allow = D - 1 - Rr - (uint32_t)rem;
+        const uint32_t dbase = sigma + b * D;  // tile-local index of domain-local 0 (before wrap)
+
+        for (uint32_t a = 0; a < A; ++a) {
+            const uint32_t slot = slot0 + k * A + a;
+            // C4: MISC block: Fm = ~lo, x2 -> position.
+            const U4 misc = philox4x32_10(slot, t, w, STREAM_MISC, P.rk);
+            int32_t x = 1 + (int32_t)mulhi32(misc.x2, n_allow);
+            if (rem > 0 && x >= lo) x += rem;
+            uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
+            if (y0 >= Ts) y0 -= Ts;
+            uint64_t *q = tile + (size_t)y0 * WB + wl;
+
+            uint64_t sa = q[0], sb = q[WB], sc = q[2 * WB], se = q[3 * WB];
+            uint64_t sf = 0;
+            if constexpr (VARIANT == 1) sf = q[4 * WB];
+
+            // C6 / Alg. 2, branch-free over the 64 replicas.
+            const uint64_t Dm = lazy_mask<STREAM_DIFF>(sb | sc, P.thd, slot, t, w, P.rk);
+            uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
+            if constexpr (VARIANT == 1) react &= se;
+            const uint64_t Pm = lazy_mask<STREAM_ANNI>(react, P.thp, slot, t, w, P.rk);
+            const uint64_t Fm = ~lo64(misc);  // 1 -> fission low (Alg. 1: r3 < 1/2)
+            uint64_t nb = (Dm & sc) | (~Dm & sb);
+            uint64_t nc = (Dm & sb) | (~Dm & sc);
+            const uint64_t ann = react & Pm;
+            const uint64_t fis = react & ~Pm;
+            nb &= ~ann;
+            nc &= ~ann;
+            sa |= fis & Fm;
+            if constexpr (VARIANT == 0) {
+                se |= fis & ~Fm;
+            } else {
+                se &= ~ann;
+                sf |= fis & ~Fm;
+                q[4 * WB] = sf;
+            }
+            q[0] = sa;
+            q[WB] = nb;
+            q[2 * WB] = nc;
+            q[3 * WB] = se;
+        }
+        __syncthreads();
+    }
+
+    // store the tile
+    if constexpr (WB >= 2) {
+        constexpr uint32_t CPR = WB / 2;
+        ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
+        const ulonglong2 *t2 = reinterpret_cast<const ulonglong2 *>(tile);
+        for (uint32_t c = tid; c < Ts * CPR; c += nthr) {
+            uint32_t i = start + c / CPR;
+            if (i >= L) i -= L;
+            g2[(size_t)i * CPR + c % CPR] = t2[c];
+        }
+    } else {
+        for (uint32_t y = tid; y < Ts; y += nthr) {
+            uint32_t i = start + y;
+            if (i >= L) i -= L;
+            g[i] = tile[y];
+        }
+    }
+}
+
+size_t sweep_smem_bytes(uint32_t Ts, int Wb) { return (size_t)Ts * Wb * 8; }
+
+template <int VARIANT, int WB>
+static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
+{
+    dim3 grid(P.L / P.Ts, P.W / WB);
+    dim3 block(P.n * WB);
+    sweep_kernel<VARIANT, WB><<<grid, block, sweep_smem_bytes(P.Ts, WB), stream>>>(P);
+    return 1;
+}
+
+int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream)
+{
+    if (variant == 0) {
+        if (Wb == 4) return launch_sweep_t<0, 4>(P, stream);
+        if (Wb == 2) return launch_sweep_t<0, 2>(P, stream);
+        return launch_sweep_t<0, 1>(P, stream);
+    }
+    if (Wb == 4) return launch_sweep_t<1, 4>(P, stream);
+    if (Wb == 2) return launch_sweep_t<1, 2>(P, stream);
+    return launch_sweep_t<1, 1>(P, stream);
+}
+
+template <int VARIANT, int WB>
+static cudaError_t cfg_one()
+{
+    return cudaFuncSetAttribute(sweep_kernel<VARIANT, WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
+int configure_kernels()
+{
+    cudaError_t e;
+    if ((e = cfg_one<0, 4>()) != cudaSuccess) return (int)e;
+    if ((e = cfg_one<0, 2>()) != cudaSuccess) return (int)e;
+    if ((e = cfg_one<0, 1>()) != cudaSuccess) return (int)e;
+    if ((e = cfg_one<1, 4>()) != cudaSuccess) return (int)e;
+    if ((e = cfg_one<1, 2>()) != cudaSuccess) return (int)e;
+    if ((e = cfg_one<1, 1>()) != cudaSuccess) return (int)e;
+    return 0;
+}
+
+}  // namespace pcpd

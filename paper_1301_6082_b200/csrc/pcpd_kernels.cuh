@@ -1,0 +1,49 @@
+// Kernel-side declarations shared by pcpd_kernels.cu (device code) and
+// pcpd_api.cu (host C ABI).  Product path only; nothing here is used by oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "philox.cuh"
+
+namespace pcpd {
+
+constexpr uint32_t MAX_SUBSTEPS = 256;  // S = D / A
+
+// One Bernoulli threshold (C3): T = floor(q * 2^32) in [0, 2^32].
+struct Threshold {
+    uint32_t T32;      // low 32 bits of T (0 when T == 2^32)
+    uint32_t nplanes;  // 32 - ctz(T): planes that can matter; 0 if T == 0 or T == 2^32
+    uint32_t all;      // 1 if T == 2^32 (mask = all ones)
+    uint32_t pad;
+};
+
+struct SweepParams {
+    uint64_t *lat;  // device, word-blocked [W/Wb][L][Wb]
+    uint32_t L, W;  // W = local word columns of this handle
+    uint32_t Ts, D, A, S, n;  // n = Ts / D domains per tile, S = D / A sub-steps
+    uint32_t word_offset;     // global index of local column 0
+    uint32_t t;               // sweep index
+    uint32_t pad;
+    Threshold thd, thp;
+    RoundKeys rk;
+};
+
+// Launchers (all asynchronous on `stream`); return the number of kernels launched.
+int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream);
+int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,
+                const RoundKeys &rk, cudaStream_t stream);
+// counts[64*w + j] (device, uint32[64*W]) must be zero on entry; pairs != 0 counts q(i) & q(i+1).
+int launch_density(const uint64_t *lat, uint32_t L, uint32_t W, int Wb, int pairs, uint32_t *counts_dev,
+                   cudaStream_t stream);
+// canonical [L][W] <-> word-blocked [W/Wb][L][Wb]
+int launch_permute(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int Wb, int to_physical,
+                   cudaStream_t stream);
+// Opt-in shared memory size etc.; returns cudaError_t as int.
+int configure_kernels();
+size_t sweep_smem_bytes(uint32_t Ts, int Wb);
+
+// microbenchmarks (microbench.cu)
+int run_microbench(int kind, uint32_t iters, double *out_rate, cudaStream_t stream);
+
+}  // namespace pcpd

@@ -1,0 +1,220 @@
+"""GPU <-> oracle parity, through the C ABI (binding = argument marshalling only).
+
+Bar: BIT-EXACT - every packed lattice word and every per-replica count equal
+to the oracle's on the same seeded inputs (integer / bit work, no tolerance).
+Scaled-down cases span several tiles, word groups of every width (Wb = 1, 2, 4),
+ragged shapes, the seam domain and the threshold edge cases; the BASELINE.json
+configs are checked in the launch configuration bench.py times, on sampled
+word columns the oracle can compute one by one (columns never interact,
+oracle pin P7), per the protocol of SURVEY.md 8(d).
+"""
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+NCPU = max(1, min(32, os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import paper_1301_6082_b200 as pk
+    from paper_1301_6082_b200 import build
+
+    build.build()
+    return pk
+
+
+def oracle_columns(cfg_kw, words, init, n_sweeps_list, words_in=None):
+    """Run the oracle on word columns `words` (one thread per column; ctypes
+    releases the GIL).  Returns {t: (lattice[L, len(words)], counts[len(words)*64])}."""
+    def one(w):
+        o = oracle.Oracle(words=[w], **cfg_kw)
+        if words_in is not None:
+            o.set_words(words_in[:, [w]])
+        else:
+            o.init(init)
+        res, prev = {}, 0
+        for t in n_sweeps_list:
+            o.run(t - prev)
+            prev = t
+            res[t] = (o.get_words()[:, 0].copy(), o.counts().copy())
+        return res
+
+    with ThreadPoolExecutor(NCPU) as ex:
+        cols = list(ex.map(one, words))
+    out = {}
+    for t in n_sweeps_list:
+        out[t] = (np.stack([c[t][0] for c in cols], axis=1), np.concatenate([c[t][1] for c in cols]))
+    return out
+
+
+def gpu_check(pk, kw, sch, init, times, words=None, words_in=None):
+    W = kw["n_replicas"] // 64
+    words = list(range(W)) if words is None else words
+    okw = dict(kw)
+    g = pk.Pcpd(kw["L"], kw["n_replicas"], kw["d"], kw["p"], kw["seed"], kw["variant"], **sch)
+    info = g.schedule_info()
+    ref = oracle_columns(dict(okw, Ts=info["Ts"], D=info["D"], A=info["A"]), words, init, times, words_in)
+    if words_in is not None:
+        g.set_lattice(words_in)
+    else:
+        g.init(init)
+    prev = 0
+    for t in times:
+        g.run(t - prev)
+        prev = t
+        lat = g.get_lattice()
+        cnt = g.density()
+        rl, rc = ref[t]
+        assert np.array_equal(lat[:, words], rl), f"lattice mismatch after sweep {t}"
+        assert np.array_equal(cnt.reshape(W, 64)[words].ravel(), rc), f"count mismatch after sweep {t}"
+        # counts agree with the lattice the GPU itself returned (all columns)
+        bits = (lat[:, :, None] >> np.arange(64, dtype=np.uint64)) & np.uint64(1) if lat.size <= (1 << 18) else None
+        if bits is not None:
+            assert np.array_equal(bits.sum(axis=0).ravel().astype(np.uint32), cnt)
+    assert g.sweep == times[-1]
+    g.close()
+
+
+def test_thresholds_and_schedule_match_oracle(pk):
+    for c in wl.CONFIGS:
+        g = pk.Pcpd(4096, 64, c.d, c.p, c.seed, c.variant)
+        o = oracle.Oracle(4096, 64, c.d, c.p, c.seed, c.variant)
+        assert g.thresholds() == o.thresholds()
+        assert g.schedule_info() == dict(Ts=2048, D=64, A=4, K=32)
+        g.close()
+
+
+SMALL = [
+    # (variant, L, R, d, p, Ts, D, A, init)            what it exercises
+    (0, 1024, 64, 0.5, 0.15, 2048, 64, 4, 0),        # W=1 (Wb=1), T_s clamped to L, d = 1/2
+    (0, 4096, 256, 0.1, 0.09, 2048, 64, 4, 1),       # W=4 (Wb=4), two tiles, generic d and p
+    (0, 8192, 128, 0.8, 0.12, 2048, 64, 4, 0),       # W=2 (Wb=2)
+    (0, 2048, 192, 0.3, 0.2, 512, 64, 8, 1),         # W=3 (Wb=1), 4 tiles, A=8
+    (0, 640, 320, 0.25, 0.75, 128, 32, 2, 1),        # W=5, ragged L = 5 tiles of 128
+    (0, 384, 512, 0.5, 0.15, 64, 64, 64, 0),         # degenerate schedule T_s = D = A (n=1, S=1)
+    (0, 112, 64, 0.37, 0.21, 56, 7, 1, 1),           # smallest legal PCPD domain D = 7
+    (1, 4096, 256, 0.5, 0.05, 2048, 64, 4, 0),       # TCPD, cfg5 shape
+    (1, 1152, 128, 0.2, 0.3, 576, 9, 3, 1),          # TCPD, smallest legal domain D = 9
+    (1, 2048, 768, 0.6, 0.1, 1024, 128, 16, 1),      # TCPD, W=12, D=128
+    (0, 1024, 128, 0.0, 0.3, 512, 64, 4, 1),         # d = 0 (T_d = 0)
+    (0, 1024, 128, 1.0, 0.3, 512, 64, 4, 1),         # d = 1 (T_d = 2^32): only swaps
+    (0, 1024, 128, 0.4, 0.0, 512, 64, 4, 1),         # p = 0: no annihilation
+    (0, 1024, 128, 0.4, 1.0, 512, 64, 4, 1),         # p = 1: every reacting pair annihilates
+    (0, 1024, 128, 2.0 ** -32, 1 - 2.0 ** -32, 512, 64, 4, 1),  # T = 1 and T = 2^32 - 1: all 32 planes matter
+]
+
+
+@pytest.mark.parametrize("case", SMALL, ids=[f"case{i}" for i in range(len(SMALL))])
+def test_small_cases_bit_exact_every_sweep(pk, case):
+    variant, L, R, d, p, Ts, D, A, init = case
+    kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
+    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)))
+
+
+def test_hand_built_lattice_and_seed_high_bits(pk):
+    L, R = 2048, 256
+    w0 = wl.random_lattice_words(L, R // 64, 0.3, seed=77)
+    kw = dict(L=L, n_replicas=R, d=0.45, p=0.13, seed=0xDEADBEEF12345678, variant=0)
+    gpu_check(pk, kw, dict(Ts=1024, D=64, A=4), None, [1, 2, 5], words_in=w0)
+
+
+def test_invariants_on_gpu(pk):
+    # absorbing state, d = 1 conservation, run splitting, set/get round trip, pair counts
+    g = pk.Pcpd(4096, 256, 0.4, 0.2, 5, 0)
+    g.init(pk.INIT_EMPTY)
+    g.run(3)
+    assert not g.get_lattice().any() and not g.density().any()
+    g.close()
+    g = pk.Pcpd(4096, 256, 1.0, 0.2, 5, 0)
+    w0 = wl.random_lattice_words(4096, 4, 0.4, seed=1)
+    g.set_lattice(w0)
+    assert np.array_equal(g.get_lattice(), w0)
+    c0 = g.density()
+    g.run(4)
+    assert np.array_equal(g.density(), c0) and not np.array_equal(g.get_lattice(), w0)
+    g.close()
+    a = pk.Pcpd(4096, 256, 0.3, 0.1, 9, 0)
+    b = pk.Pcpd(4096, 256, 0.3, 0.1, 9, 0)
+    a.init(1)
+    b.init(1)
+    a.run(7)
+    b.run(3)
+    b.run(4)
+    assert np.array_equal(a.get_lattice(), b.get_lattice())
+    lat = a.get_lattice()
+    pairs = ((lat & np.roll(lat, -1, axis=0))[:, :, None] >> np.arange(64, dtype=np.uint64)) & np.uint64(1)
+    assert np.array_equal(a.pair_density(), pairs.sum(axis=0).ravel().astype(np.uint32))
+    o = oracle.Oracle(4096, 256, 0.3, 0.1, 9, 0)
+    o.set_words(lat)
+    assert np.array_equal(a.pair_density(), o.pair_counts())
+    # checkpoint / resume: lattice + sweep counter is the whole state (C7)
+    c = pk.Pcpd(4096, 256, 0.3, 0.1, 9, 0)
+    c.set_lattice(b.get_lattice())
+    c.sweep = 7
+    a.run(2)
+    c.run(2)
+    assert np.array_equal(a.get_lattice(), c.get_lattice())
+    for h in (a, b, c):
+        h.close()
+
+
+def test_word_offset_shards_equal_one_big_run(pk):
+    kw = dict(d=0.3, p=0.12, seed=31, variant=0)
+    big = pk.Pcpd(2048, 512, **kw)
+    big.init(1)
+    big.run(3)
+    full = big.get_lattice()
+    for rank in range(2):
+        w0, w1 = pk.shard_words(8, 2, rank)
+        s = pk.Pcpd(2048, 64 * (w1 - w0), **kw, word_offset=w0)
+        s.init(1)
+        s.run(3)
+        assert np.array_equal(s.get_lattice(), full[:, w0:w1])
+        assert np.array_equal(s.density(), big.density()[64 * w0:64 * w1])
+        s.close()
+    big.close()
+
+
+def test_cfg1_every_sweep(pk):
+    c = wl.BY_NAME["cfg1"]
+    kw = dict(L=c.L, n_replicas=c.n_replicas, d=c.d, p=c.p, seed=c.seed, variant=c.variant)
+    gpu_check(pk, kw, {}, c.init, list(range(1, c.sweeps + 1)))
+
+
+def test_cfg2_prefix(pk):
+    c = wl.BY_NAME["cfg2"]
+    kw = dict(L=c.L, n_replicas=c.n_replicas, d=c.d, p=c.p, seed=c.seed, variant=c.variant)
+    horizon = 32 if NCPU >= 4 else 8
+    times = [t for t in wl.record_times(c.sweeps) if 0 < t <= horizon]
+    gpu_check(pk, kw, {}, c.init, times)
+
+
+@pytest.mark.parametrize("name,words,horizon", [("cfg3", [0, 16, 31], 4), ("cfg5", [0, 8, 15], 4), ("cfg4", [0, 31], 2)])
+def test_full_size_configs_sampled_columns(pk, name, words, horizon):
+    """Full BASELINE sizes in the launch configuration bench.py times; the
+    oracle computes the sampled word columns one by one."""
+    c = wl.BY_NAME[name]
+    kw = dict(L=c.L, n_replicas=c.n_replicas, d=c.d, p=c.p, seed=c.seed, variant=c.variant)
+    times = [t for t in (1, 2, 4) if t <= horizon]
+    gpu_check(pk, kw, {}, c.init, times, words=words)
+
+
+def test_philox_block_via_init_stream(pk):
+    """The device Philox against the KAT-pinned oracle block function on the
+    INIT stream (C8), 2^16 blocks with seed words in both key halves."""
+    seed = 0x0123456789ABCDEF
+    g = pk.Pcpd(16384, 256, 0.5, 0.1, seed, 0, word_offset=1000)
+    g.init(pk.INIT_BERNOULLI)
+    lat = g.get_lattice()
+    o = oracle.Oracle(16384, 64 * 1004, 0.5, 0.1, seed, 0, words=[1000, 1001, 1002, 1003])
+    o.init(wl.INIT_BERNOULLI)
+    assert np.array_equal(lat, o.get_words())
+    g.close()

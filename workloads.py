@@ -101,11 +101,3 @@ def isolated_particles_words(L: int, W: int, spacing: int, seed: int) -> np.ndar
             off = int(rng.integers(0, spacing))
             out[off::spacing, w] |= np.uint64(1) << np.uint64(j)
     return out
-
-
-def shard_words(W: int, world_size: int, rank: int) -> tuple[int, int]:
-    """Word-column shard [w0, w1) of rank `rank`: columns never
-    interact, so the union over ranks is bit-identical to the 1-GPU run."""
-    base, extra = divmod(W, world_size)
-    w0 = rank * base + min(rank, extra)
-    return w0, w0 + base + (1 if rank < extra else 0)
