@@ -10,8 +10,10 @@ Names follow the C ABI: pcpd_create / pcpd_init / pcpd_run / pcpd_density ...
 """
 from __future__ import annotations
 
+import atexit
 import ctypes as C
 import os
+import weakref
 
 import numpy as np
 
@@ -37,6 +39,16 @@ _FREE_FN = C.CFUNCTYPE(None, C.c_void_p)
 
 _lib = None
 _keepalive = []
+_live = weakref.WeakSet()  # open handles; closed at interpreter exit while torch's allocator is still alive
+
+
+@atexit.register
+def _close_all():
+    for h in list(_live):
+        try:
+            h.close()
+        except Exception:
+            pass
 
 
 class PcpdError(RuntimeError):
@@ -157,6 +169,7 @@ class Pcpd:
         if not h:
             raise PcpdError(f"pcpd_create failed: {_err(lib)}")
         self._h = h
+        _live.add(self)
         self.L, self.n_replicas, self.W = int(L), int(n_replicas), int(n_replicas) // 64
         self.use_current_stream()
 

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpcpd.so")
-SOURCES = ["pcpd_api.cu", "pcpd_kernels.cu", "pcpd_aux.cu", "microbench.cu"]
+SOURCES = ["pcpd_api.cu", "pcpd_kernels.cu", "sweep_warp.cu", "pcpd_aux.cu", "microbench.cu"]
 HEADERS = ["philox.cuh", "pcpd_kernels.cuh", os.path.join("..", "..", "include", "pcpd.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -138,16 +138,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_ARG, "schedule: D / A must be <= %u", MAX_SUBSTEPS);
         return nullptr;
     }
-    // word-group width: widest of 4, 2, 1 dividing W that fits shared memory / block size
-    int Wb = 1;
-    for (int cand = 4; cand >= 1; cand >>= 1) {
-        if (W % cand) continue;
-        if (sweep_smem_bytes(Ts, cand) > 200 * 1024) continue;
-        if ((uint64_t)(Ts / D) * cand > 1024) continue;
-        Wb = cand;
-        break;
-    }
-    if (sweep_smem_bytes(Ts, Wb) > 200 * 1024 || (uint64_t)(Ts / D) * Wb > 1024) {
+    // Physical layout: column-major [W][L] (word-group width Wb = 1): a tile column is one
+    // contiguous run of T_s words, which is what the warp-per-(tile, column) sweep kernel loads.
+    const int Wb = 1;
+    if (!sweep_warp_supported(Ts, D) && (sweep_smem_bytes(Ts, Wb) > 200 * 1024 || (uint64_t)(Ts / D) > 1024)) {
         fail(PCPD_ERR_ARG, "schedule: tile of %u sites does not fit one thread block", Ts);
         return nullptr;
     }

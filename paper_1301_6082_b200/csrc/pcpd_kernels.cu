@@ -179,6 +179,7 @@ static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
 
 int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream)
 {
+    if (Wb == 1 && sweep_warp_supported(P.Ts, P.D)) return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts), stream);
     if (variant == 0) {
         if (Wb == 4) return launch_sweep_t<0, 4>(P, stream);
         if (Wb == 2) return launch_sweep_t<0, 2>(P, stream);
@@ -204,7 +205,7 @@ int configure_kernels()
     if ((e = cfg_one<1, 4>()) != cudaSuccess) return (int)e;
     if ((e = cfg_one<1, 2>()) != cudaSuccess) return (int)e;
     if ((e = cfg_one<1, 1>()) != cudaSuccess) return (int)e;
-    return 0;
+    return configure_warp_kernels();
 }
 
 }  // namespace pcpd

@@ -31,6 +31,11 @@ struct SweepParams {
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.
 int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream);
+// warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
+bool sweep_warp_supported(uint32_t Ts, uint32_t D);
+int sweep_warp_wpb(uint32_t Ts);
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream);
+int configure_warp_kernels();
 int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,
                 const RoundKeys &rk, cudaStream_t stream);
 // counts[64*w + j] (device, uint32[64*W]) must be zero on entry; pairs != 0 counts q(i) & q(i+1).

@@ -1,0 +1,457 @@
+// sweep_warp_kernel - the production sweep kernel for sm_100a.
+//
+// Mapping: ONE WARP owns one (tile, word column) for a whole sweep; LANE b owns
+// domain b of that tile (n = T_s / D <= 32 domains).  The column's T_s words
+// live in shared memory from load to store, so the lattice crosses HBM exactly
+// once in each direction per sweep (0.25 B per replica-site update), with
+// coalesced 128-bit global accesses.  Because all domains of a tile column sit
+// in one warp, sub-steps need __syncwarp() only - no block barrier anywhere in
+// the sweep.
+//
+// Per sub-step the A attempts of a lane are processed in batches of NB:
+//   phase A (state-independent, so batched over the NB attempts for ILP):
+//           MISC block -> position x, fission-side mask Fm;
+//           DIFF planes -> Dm on all 64 lanes, NU_D blocks unconditionally,
+//           then lazily while any lane of the warp is undecided;
+//   phase B (sequential in a): load the footprint, react = pair & ~Dm, ANNI
+//           planes lazily on the react lanes only, bitwise rule, store.
+// Philox rounds 1-3 are strength-reduced: the products that depend only on
+// (w, t) or only on the slot are computed once per warp / once per attempt,
+// leaving 16 IMAD.WIDE.U32 per block instead of 20.
+//
+// Citations: update rule = Alg. 1 PAPER.md:45-70 in the bitwise form of Alg. 2
+// PAPER.md:126-151 (typos fixed per DESIGN.md readings G5/G6); schedule SD2 and
+// streams = DESIGN.md section 3 C1-C9.
+#include "pcpd_kernels.cuh"
+
+namespace pcpd {
+
+namespace {
+
+__device__ __forceinline__ uint32_t hi32(uint64_t v) { return (uint32_t)(v >> 32); }
+__device__ __forceinline__ uint32_t lo32(uint64_t v) { return (uint32_t)v; }
+__device__ __forceinline__ uint64_t mulw(uint32_t a, uint32_t b) { return (uint64_t)a * b; }
+
+// Constants of one (sweep t, word w) pair: everything in rounds 1-3 that does
+// not depend on the slot or on c3.
+struct PhiloxWarp {
+    uint32_t B;     // lo(M1 w) ^ k0[1]
+    uint32_t C;     // hi(M0 c0') ^ k1[1],  c0' = hi(M1 w) ^ t ^ k0[0]
+    uint32_t Dc;    // lo(M0 c0') ^ k1[2]
+};
+
+__device__ __forceinline__ PhiloxWarp philox_warp_consts(uint32_t t, uint32_t w, const RoundKeys &rk)
+{
+    const uint64_t p1 = mulw(PHILOX_M1, w);
+    const uint32_t c0p = hi32(p1) ^ t ^ rk.k0[0];
+    const uint64_t p0p = mulw(PHILOX_M0, c0p);
+    PhiloxWarp pw;
+    pw.B = lo32(p1) ^ rk.k0[1];
+    pw.C = hi32(p0p) ^ rk.k1[1];
+    pw.Dc = lo32(p0p) ^ rk.k1[2];
+    return pw;
+}
+
+// Constants of one slot (attempt): 2 wide multiplies.
+struct PhiloxSlot {
+    uint32_t X;    // hi(M0 slot) ^ k1[0]           (c2' = X ^ c3)
+    uint32_t E;    // hi(M1 c2'') ^ k0[2],  c2'' = C ^ lo(M0 slot)
+    uint32_t c1;   // lo(M1 c2'')                    (c1 entering round 4)
+};
+
+__device__ __forceinline__ PhiloxSlot philox_slot_consts(uint32_t slot, const PhiloxWarp &pw, const RoundKeys &rk)
+{
+    const uint64_t p0 = mulw(PHILOX_M0, slot);
+    const uint32_t c2pp = pw.C ^ lo32(p0);
+    const uint64_t p1pp = mulw(PHILOX_M1, c2pp);
+    PhiloxSlot ps;
+    ps.X = hi32(p0) ^ rk.k1[0];
+    ps.E = hi32(p1pp) ^ rk.k0[2];
+    ps.c1 = lo32(p1pp);
+    return ps;
+}
+
+// Philox-4x32-10 block of counter (slot, t, w, c3): 16 IMAD.WIDE.U32 + 18 LOP3.
+__device__ __forceinline__ U4 philox_block(uint32_t c3, const PhiloxSlot &ps, const PhiloxWarp &pw,
+                                           const RoundKeys &rk)
+{
+    // round 1 -> only c2' depends on c3; round 2: one multiply; round 3: one multiply
+    const uint32_t c2p = ps.X ^ c3;
+    const uint64_t p1p = mulw(PHILOX_M1, c2p);
+    const uint32_t c0pp = hi32(p1p) ^ pw.B;
+    const uint64_t p0pp = mulw(PHILOX_M0, c0pp);
+    uint32_t c0 = ps.E ^ lo32(p1p);
+    uint32_t c1 = ps.c1;
+    uint32_t c2 = hi32(p0pp) ^ pw.Dc;
+    uint32_t c3r = lo32(p0pp);
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+        const uint64_t p0 = mulw(PHILOX_M0, c0);
+        const uint64_t p1 = mulw(PHILOX_M1, c2);
+        const uint32_t n0 = hi32(p1) ^ c1 ^ rk.k0[r];
+        const uint32_t n2 = hi32(p0) ^ c3r ^ rk.k1[r];
+        c1 = lo32(p1);
+        c3r = lo32(p0);
+        c0 = n0;
+        c2 = n2;
+    }
+    return U4{c0, c1, c2, c3r};
+}
+
+// N blocks of one slot at once, written round-major / chain-minor so that the N
+// independent multiply chains are interleaved in the instruction stream (ptxas
+// keeps source order within its window; block-after-block code leaves the FMA
+// pipe waiting on one chain's latency).
+template <int N>
+__device__ __forceinline__ void philox_blocks(const uint32_t (&c3in)[N], const PhiloxSlot &ps, const PhiloxWarp &pw,
+                                              const RoundKeys &rk, U4 *out)
+{
+    uint32_t c0[N], c1[N], c2[N], c3[N];
+    uint64_t pa[N], pb[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) pa[i] = mulw(PHILOX_M1, ps.X ^ c3in[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) pb[i] = mulw(PHILOX_M0, hi32(pa[i]) ^ pw.B);
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        c0[i] = ps.E ^ lo32(pa[i]);
+        c1[i] = ps.c1;
+        c2[i] = hi32(pb[i]) ^ pw.Dc;
+        c3[i] = lo32(pb[i]);
+    }
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            pa[i] = mulw(PHILOX_M0, c0[i]);
+            pb[i] = mulw(PHILOX_M1, c2[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            c0[i] = hi32(pb[i]) ^ c1[i] ^ rk.k0[r];
+            c2[i] = hi32(pa[i]) ^ c3[i] ^ rk.k1[r];
+            c1[i] = lo32(pb[i]);
+            c3[i] = lo32(pa[i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) out[i] = U4{c0[i], c1[i], c2[i], c3[i]};
+}
+
+// MSB-first bit-sliced compare of two planes (p0 = plane 2m, p1 = plane 2m+1)
+// against T's two bits for those planes, given as all-ones / all-zeros masks
+// tb0, tb1 (C3), on one 32-lane half of the word.  Branch-free (5 LOP3), so that
+// an attempt's unconditional blocks form one basic block.
+__device__ __forceinline__ void cmp2h(uint32_t &lt, uint32_t &und, uint32_t p0, uint32_t p1, uint32_t tb0,
+                                      uint32_t tb1)
+{
+    const uint32_t u1 = und & ~(p0 ^ tb0);       // still equal to T after plane 2m
+    const uint32_t a = und & ~p0 & tb0;          // decided at plane 2m: lane bit 0, T bit 1 -> U < T
+    const uint32_t b = u1 & ~p1 & tb1;           // decided at plane 2m+1
+    und = u1 & ~(p1 ^ tb1);
+    lt |= a | b;
+}
+
+// 64-lane mask state as two 32-bit halves.
+struct Mask2 {
+    uint32_t lo, hi;
+};
+__device__ __forceinline__ uint64_t m64(const Mask2 &m) { return (uint64_t)m.lo | ((uint64_t)m.hi << 32); }
+
+// block blk = planes 2m (x0 | x1 << 32) and 2m+1 (x2 | x3 << 32)
+__device__ __forceinline__ void cmp_block(Mask2 &lt, Mask2 &und, const U4 &blk, uint32_t tb0, uint32_t tb1)
+{
+    cmp2h(lt.lo, und.lo, blk.x0, blk.x2, tb0, tb1);
+    cmp2h(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1);
+}
+
+// T's bit for plane k (bit 31-k) as a 32-lane mask.
+__device__ __forceinline__ uint32_t tmask(uint32_t T32, uint32_t k)
+{
+    return 0u - ((T32 >> (31u - k)) & 1u);
+}
+
+// Copy of a grid-uniform value in a vector register, opaque to the optimiser:
+// stops ptxas from re-loading / re-deriving it on the uniform datapath inside the
+// attempt loop (those instructions cost issue slots the Philox rounds need).
+__device__ __forceinline__ uint32_t vreg(uint32_t v)
+{
+    uint32_t r;
+    asm volatile("mov.b32 %0, %1;" : "=r"(r) : "r"(v));
+    return r;
+}
+
+}  // namespace
+
+// NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
+// parameters so that the unconditional part has no branch at all).  A warp needs DIFF block 3
+// w.p. > 0.999 when the threshold has >= 8 planes, so NU_D = 4 there; ANNI matters only on the
+// reacting lanes (a few per word), so NU_P = 2.  Thresholds with fewer planes get fewer blocks.
+template <int VARIANT, int WPB, int NU_D, int NU_P>
+__global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
+{
+    extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
+
+    constexpr uint32_t Rr = VARIANT == 0 ? 2u : 3u;
+    const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t ntiles = L / Ts;
+    const uint32_t task = blockIdx.x * WPB + warp;
+    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel
+
+    // C5 step 1: shifts from the SHIFT stream; lane j holds sigma_{k0+j} of the current group of 32 sub-steps.
+    uint32_t sig_reg, Sigma;
+    {
+        const U4 blk = philox4x32_10(lane, t, 0u, STREAM_SHIFT, P.rk);
+        sig_reg = __umulhi(blk.x0, D);
+        Sigma = __shfl_sync(0xffffffffu, __umulhi(blk.x1, Ts), 0);
+    }
+    const uint32_t tau = task % ntiles, wl = task / ntiles;
+    const uint32_t w = P.word_offset + wl;  // global word index (RNG key)
+
+    // ---- C5 step 2: tile tau covers global sites (Sigma + tau*Ts + y) mod L ----
+    const uint32_t start = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts) % L);
+    uint64_t *g = P.lat + (size_t)wl * L;             // column wl, contiguous in the site index
+    const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
+    uint64_t *buf = smem + (size_t)warp * stride;
+    const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
+    const uint32_t odd = vec ? (start & 1u) : 0u;
+    uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
+    if (vec) {
+        const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
+        const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
+        ulonglong2 *b2 = reinterpret_cast<ulonglong2 *>(buf);
+#pragma unroll 8
+        for (uint32_t pi = lane; pi < npairs; pi += 32) {
+            uint32_t i = s0 + 2 * pi;
+            if (i >= L) i -= L;
+            b2[pi] = g2[i >> 1];
+        }
+    } else {
+        for (uint32_t y = lane; y < Ts; y += 32) {
+            uint32_t i = start + y;
+            if (i >= L) i -= L;
+            tile[y] = g[i];
+        }
+    }
+    __syncwarp();
+
+    const PhiloxWarp pw = philox_warp_consts(t, w, P.rk);
+    // Loop constants held in vector registers (see vreg): round keys of rounds 4-10 and the slot
+    // constants' keys, and T's bits for the unconditional planes.
+    RoundKeys rkv;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        rkv.k0[r] = vreg(P.rk.k0[r]);
+        rkv.k1[r] = vreg(P.rk.k1[r]);
+    }
+    uint32_t tdm[2 * NU_D + 1], tpm[2 * NU_P + 1];
+#pragma unroll
+    for (int kk = 0; kk < 2 * NU_D; ++kk) tdm[kk] = vreg(tmask(P.thd.T32, kk));
+#pragma unroll
+    for (int kk = 0; kk < 2 * NU_P; ++kk) tpm[kk] = vreg(tmask(P.thp.T32, kk));
+    const bool act = lane < n;
+    const uint32_t b = act ? lane : 0u;
+    const uint32_t slot0 = (tau * n + b) * D;
+    const uint32_t nblkD = (P.thd.nplanes + 1u) >> 1, nblkP = (P.thp.nplanes + 1u) >> 1;
+    const uint32_t Td = P.thd.T32, Tp = P.thp.T32;
+
+    for (uint32_t k = 0; k < S; ++k) {
+        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, P.rk).x0, D);
+        const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
+        // C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
+        // domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
+        const bool seam = (b == n - 1) && (sigma > 0);
+        const int32_t c = (int32_t)D - (int32_t)sigma;
+        int32_t lo = 0, rem = 0;
+        if (seam) {
+            lo = max(1, c - (int32_t)Rr);
+            const int32_t hi = min((int32_t)D - 1 - (int32_t)Rr, c);
+            rem = max(0, hi - lo + 1);
+        }
+        const uint32_t n_allow = D - 1 - Rr - (uint32_t)rem;
+        const uint32_t dbase = sigma + b * D;  // tile-local index of domain-local 0 (before wrap)
+
+        for (uint32_t a = 0; a < A; ++a) {
+            // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
+            // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
+            // back to back so that the FMA pipe always has several wide multiplies in flight.
+            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, rkv);
+            uint32_t c3s[1 + NU_D + NU_P];
+            U4 blks[1 + NU_D + NU_P];
+            c3s[0] = STREAM_MISC;
+#pragma unroll
+            for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
+#pragma unroll
+            for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
+            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, rkv, blks);
+            const U4 misc = blks[0];
+            const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
+
+            // C4: MISC block: Fm = ~lo (1 -> fission low, Alg. 1: r3 < 1/2), x2 -> position.
+            int32_t x = 1 + (int32_t)__umulhi(misc.x2, n_allow);
+            if (rem > 0 && x >= lo) x += rem;
+            uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
+            if (y0 >= Ts) y0 -= Ts;
+            const uint64_t Fm = ~lo64(misc);
+
+            // DIFF mask on all 64 lanes (C3), lazily beyond the first NU_D blocks.
+            Mask2 dlt{0u, 0u}, dund{act ? ~0u : 0u, act ? ~0u : 0u};
+#pragma unroll
+            for (int m = 0; m < NU_D; ++m) cmp_block(dlt, dund, dblk[m], tdm[2 * m], tdm[2 * m + 1]);
+            if (NU_D < 16) {
+                uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top
+                for (uint32_t m = NU_D; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
+                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rkv);
+                    cmp_block(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
+                    Tsh <<= 2;
+                }
+            }
+
+            uint64_t *q = tile + y0;
+            uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0;
+            if (act) {
+                sa = q[0]; sb = q[1]; sc = q[2]; se = q[3];
+                if constexpr (VARIANT == 1) sf = q[4];
+            }
+            const uint64_t Dm = P.thd.all ? ~0ull : m64(dlt);
+            uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
+            if constexpr (VARIANT == 1) react &= se;
+
+            // ANNI mask: only the reacting lanes matter.
+            Mask2 plt{0u, 0u}, pund{(uint32_t)react, (uint32_t)(react >> 32)};
+#pragma unroll
+            for (int m = 0; m < NU_P; ++m) cmp_block(plt, pund, pblk[m], tpm[2 * m], tpm[2 * m + 1]);
+            {
+                uint32_t Tsh = Tp << (2 * NU_P);
+                for (uint32_t m = NU_P; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
+                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rkv);
+                    cmp_block(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
+                    Tsh <<= 2;
+                }
+            }
+            const uint64_t Pm = P.thp.all ? ~0ull : m64(plt);
+
+            // C6 / Alg. 2, branch-free over the 64 replicas.
+            uint64_t nb = (Dm & sc) | (~Dm & sb);
+            uint64_t nc = (Dm & sb) | (~Dm & sc);
+            const uint64_t ann = react & Pm;
+            const uint64_t fis = react & ~Pm;
+            nb &= ~ann;
+            nc &= ~ann;
+            sa |= fis & Fm;
+            if (act) {
+                if constexpr (VARIANT == 0) {
+                    se |= fis & ~Fm;
+                } else {
+                    se &= ~ann;
+                    sf |= fis & ~Fm;
+                    q[4] = sf;
+                }
+                q[0] = sa; q[1] = nb; q[2] = nc; q[3] = se;
+            }
+        }
+        __syncwarp();
+    }
+
+    // ---- store the tile ----
+    if (vec) {
+        const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
+        ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
+        const ulonglong2 *b2 = reinterpret_cast<const ulonglong2 *>(buf);
+#pragma unroll 8
+        for (uint32_t pi = lane; pi < npairs; pi += 32) {
+            uint32_t i = s0 + 2 * pi;
+            if (i >= L) i -= L;
+            if (odd && (pi == 0 || pi == npairs - 1)) {
+                // edge pairs of an odd-aligned tile hold one foreign word each
+                if (pi == 0) g[i + 1] = buf[1];
+                else g[i] = buf[2 * pi];
+            } else {
+                g2[i >> 1] = b2[pi];
+            }
+        }
+    } else {
+        for (uint32_t y = lane; y < Ts; y += 32) {
+            uint32_t i = start + y;
+            if (i >= L) i -= L;
+            g[i] = tile[y];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
+static size_t warp_smem_bytes(uint32_t Ts, int wpb) { return (size_t)wpb * ((Ts + 3u) & ~1u) * 8; }
+
+bool sweep_warp_supported(uint32_t Ts, uint32_t D)
+{
+    return Ts / D <= 32 && warp_smem_bytes(Ts, 1) <= 200 * 1024;
+}
+
+// warps per block: as many as fit 227 KB / SM in at most a few blocks
+int sweep_warp_wpb(uint32_t Ts)
+{
+    const size_t per = warp_smem_bytes(Ts, 1);
+    if (7 * per <= 113 * 1024) return 7;   // 2 blocks x 7 warps per SM at T_s = 2048 (2 x (114800 + 1024) B)
+    return 1;
+}
+
+// prefix lengths for a threshold with nblk blocks
+static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 4 ? 1 : 4; }
+static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 2 ? 1 : 2; }
+
+template <int VARIANT, int WPB, int NU_D, int NU_P>
+static int warp_op(const SweepParams *P, cudaStream_t stream)
+{
+    if (!P)  // configure
+        return (int)cudaFuncSetAttribute(sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         WPB >= 4 ? 116 * 1024 : 226 * 1024);
+    const uint32_t ntasks = (P->L / P->Ts) * P->W;
+    sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P>
+        <<<(ntasks + WPB - 1) / WPB, WPB * 32, warp_smem_bytes(P->Ts, WPB), stream>>>(*P);
+    return 1;
+}
+
+template <int VARIANT, int WPB, int NU_D>
+static int warp_op_p(int nup, const SweepParams *P, cudaStream_t stream)
+{
+    if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0>(P, stream);
+    if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1>(P, stream);
+    return warp_op<VARIANT, WPB, NU_D, 2>(P, stream);
+}
+
+template <int VARIANT, int WPB>
+static int warp_op_d(int nud, int nup, const SweepParams *P, cudaStream_t stream)
+{
+    if (nud == 0) return warp_op_p<VARIANT, WPB, 0>(nup, P, stream);
+    if (nud == 1) return warp_op_p<VARIANT, WPB, 1>(nup, P, stream);
+    return warp_op_p<VARIANT, WPB, 4>(nup, P, stream);
+}
+
+static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams *P, cudaStream_t stream)
+{
+    if (variant == 0) return wpb == 7 ? warp_op_d<0, 7>(nud, nup, P, stream) : warp_op_d<0, 1>(nud, nup, P, stream);
+    return wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream) : warp_op_d<1, 1>(nud, nup, P, stream);
+}
+
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
+{
+    return warp_op_any(variant, wpb, nu_d_of((P.thd.nplanes + 1) >> 1), nu_p_of((P.thp.nplanes + 1) >> 1), &P, stream);
+}
+
+int configure_warp_kernels()
+{
+    const int nuds[3] = {0, 1, 4}, nups[3] = {0, 1, 2}, wpbs[2] = {7, 1};
+    for (int variant = 0; variant < 2; ++variant)
+        for (int wpb : wpbs)
+            for (int nud : nuds)
+                for (int nup : nups) {
+                    const int e = warp_op_any(variant, wpb, nud, nup, nullptr, nullptr);
+                    if (e != 0) return e;
+                }
+    return 0;
+}
+
+}  // namespace pcpd

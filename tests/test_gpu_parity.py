@@ -102,7 +102,9 @@ SMALL = [
     (0, 384, 512, 0.5, 0.15, 64, 64, 64, 0),         # degenerate schedule T_s = D = A (n=1, S=1)
     (0, 112, 64, 0.37, 0.21, 56, 7, 1, 1),           # smallest legal PCPD domain D = 7
     (1, 4096, 256, 0.5, 0.05, 2048, 64, 4, 0),       # TCPD, cfg5 shape
-    (1, 1152, 128, 0.2, 0.3, 576, 9, 3, 1),          # TCPD, smallest legal domain D = 9
+    (1, 1152, 128, 0.2, 0.3, 576, 9, 3, 1),          # TCPD, smallest legal domain D = 9 (n = 64: generic block kernel)
+    (0, 147, 64, 0.37, 0.21, 49, 7, 1, 1),           # odd L and T_s: 64-bit tile copy path
+    (1, 4096, 128, 0.5, 0.05, 1024, 32, 2, 1),       # TCPD, n = 32 lanes, A = 2 batches
     (1, 2048, 768, 0.6, 0.1, 1024, 128, 16, 1),      # TCPD, W=12, D=128
     (0, 1024, 128, 0.0, 0.3, 512, 64, 4, 1),         # d = 0 (T_d = 0)
     (0, 1024, 128, 1.0, 0.3, 512, 64, 4, 1),         # d = 1 (T_d = 2^32): only swaps
