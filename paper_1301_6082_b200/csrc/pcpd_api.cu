@@ -196,6 +196,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     P.thd = make_threshold(h->Td);
     P.thp = make_threshold(h->Tp);
     P.rk = make_round_keys(seed);
+    for (int k = 0; k < 32; ++k) {
+        P.tdm[k] = ((P.thd.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
+        P.tpm[k] = ((P.thp.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
+    }
     g_err[0] = 0;
     return h;
 }
@@ -345,7 +349,7 @@ int pcpd_synchronize(pcpd_t *h)
 
 int pcpd_microbench(int kind, uint32_t iters, double *out_rate)
 {
-    if (kind < 0 || kind > 3 || !out_rate || iters == 0) return fail(PCPD_ERR_ARG, "microbench: bad arguments");
+    if (kind < 0 || kind > 7 || !out_rate || iters == 0) return fail(PCPD_ERR_ARG, "microbench: bad arguments");
     const int rc = run_microbench(kind, iters, out_rate, nullptr);
     g_launches += 4;
     if (rc != 0) return fail(rc, "microbench failed");

@@ -27,6 +27,9 @@ struct SweepParams {
     uint32_t pad;
     Threshold thd, thp;
     RoundKeys rk;
+    // T's bit for plane k (bit 31-k) as an all-ones / all-zeros 32-lane mask, precomputed on the
+    // host so that the kernels read them as constant-bank operands (C3)
+    uint32_t tdm[32], tpm[32];
 };
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.

@@ -171,16 +171,6 @@ __device__ __forceinline__ uint32_t tmask(uint32_t T32, uint32_t k)
     return 0u - ((T32 >> (31u - k)) & 1u);
 }
 
-// Copy of a grid-uniform value in a vector register, opaque to the optimiser:
-// stops ptxas from re-loading / re-deriving it on the uniform datapath inside the
-// attempt loop (those instructions cost issue slots the Philox rounds need).
-__device__ __forceinline__ uint32_t vreg(uint32_t v)
-{
-    uint32_t r;
-    asm volatile("mov.b32 %0, %1;" : "=r"(r) : "r"(v));
-    return r;
-}
-
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
@@ -238,19 +228,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     __syncwarp();
 
     const PhiloxWarp pw = philox_warp_consts(t, w, P.rk);
-    // Loop constants held in vector registers (see vreg): round keys of rounds 4-10 and the slot
-    // constants' keys, and T's bits for the unconditional planes.
-    RoundKeys rkv;
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        rkv.k0[r] = vreg(P.rk.k0[r]);
-        rkv.k1[r] = vreg(P.rk.k1[r]);
-    }
-    uint32_t tdm[2 * NU_D + 1], tpm[2 * NU_P + 1];
-#pragma unroll
-    for (int kk = 0; kk < 2 * NU_D; ++kk) tdm[kk] = vreg(tmask(P.thd.T32, kk));
-#pragma unroll
-    for (int kk = 0; kk < 2 * NU_P; ++kk) tpm[kk] = vreg(tmask(P.thp.T32, kk));
     const bool act = lane < n;
     const uint32_t b = act ? lane : 0u;
     const uint32_t slot0 = (tau * n + b) * D;
@@ -277,7 +254,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
             // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
             // back to back so that the FMA pipe always has several wide multiplies in flight.
-            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, rkv);
+            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, P.rk);
             uint32_t c3s[1 + NU_D + NU_P];
             U4 blks[1 + NU_D + NU_P];
             c3s[0] = STREAM_MISC;
@@ -285,7 +262,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
 #pragma unroll
             for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
-            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, rkv, blks);
+            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, P.rk, blks);
             const U4 misc = blks[0];
             const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
 
@@ -295,38 +272,41 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
             if (y0 >= Ts) y0 -= Ts;
             const uint64_t Fm = ~lo64(misc);
-
-            // DIFF mask on all 64 lanes (C3), lazily beyond the first NU_D blocks.
-            Mask2 dlt{0u, 0u}, dund{act ? ~0u : 0u, act ? ~0u : 0u};
-#pragma unroll
-            for (int m = 0; m < NU_D; ++m) cmp_block(dlt, dund, dblk[m], tdm[2 * m], tdm[2 * m + 1]);
-            if (NU_D < 16) {
-                uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top
-                for (uint32_t m = NU_D; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
-                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rkv);
-                    cmp_block(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
-                    Tsh <<= 2;
-                }
-            }
-
             uint64_t *q = tile + y0;
             uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0;
             if (act) {
                 sa = q[0]; sb = q[1]; sc = q[2]; se = q[3];
                 if constexpr (VARIANT == 1) sf = q[4];
             }
+
+            // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
+            // dependence on the state), the lazy tails only on the lanes whose outcome can matter:
+            // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
+            Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
+#pragma unroll
+            for (int m = 0; m < NU_D; ++m) cmp_block(dlt, dund, dblk[m], P.tdm[2 * m], P.tdm[2 * m + 1]);
+#pragma unroll
+            for (int m = 0; m < NU_P; ++m) cmp_block(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1]);
+            {
+                const uint64_t rel = sb | sc;
+                dund.lo &= (uint32_t)rel;
+                dund.hi &= (uint32_t)(rel >> 32);
+                uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top (0 past the last plane)
+                for (uint32_t m = NU_D; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
+                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, P.rk);
+                    cmp_block(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
+                    Tsh <<= 2;
+                }
+            }
             const uint64_t Dm = P.thd.all ? ~0ull : m64(dlt);
             uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
             if constexpr (VARIANT == 1) react &= se;
-
-            // ANNI mask: only the reacting lanes matter.
-            Mask2 plt{0u, 0u}, pund{(uint32_t)react, (uint32_t)(react >> 32)};
-#pragma unroll
-            for (int m = 0; m < NU_P; ++m) cmp_block(plt, pund, pblk[m], tpm[2 * m], tpm[2 * m + 1]);
             {
+                pund.lo &= (uint32_t)react;
+                pund.hi &= (uint32_t)(react >> 32);
                 uint32_t Tsh = Tp << (2 * NU_P);
                 for (uint32_t m = NU_P; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
-                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rkv);
+                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, P.rk);
                     cmp_block(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
                     Tsh <<= 2;
                 }
@@ -393,13 +373,14 @@ bool sweep_warp_supported(uint32_t Ts, uint32_t D)
 int sweep_warp_wpb(uint32_t Ts)
 {
     const size_t per = warp_smem_bytes(Ts, 1);
+    if (14 * per <= 113 * 1024) return 14; // 2 blocks x 14 warps per SM at T_s = 1024 (2 x (114912 + 1024) B)
     if (7 * per <= 113 * 1024) return 7;   // 2 blocks x 7 warps per SM at T_s = 2048 (2 x (114800 + 1024) B)
     return 1;
 }
 
 // prefix lengths for a threshold with nblk blocks
-static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 4 ? 1 : 4; }
-static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 2 ? 1 : 2; }
+static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 6 ? 1 : 6; }
+static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 4 ? 1 : 4; }
 
 template <int VARIANT, int WPB, int NU_D, int NU_P>
 static int warp_op(const SweepParams *P, cudaStream_t stream)
@@ -419,7 +400,7 @@ static int warp_op_p(int nup, const SweepParams *P, cudaStream_t stream)
 {
     if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0>(P, stream);
     if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1>(P, stream);
-    return warp_op<VARIANT, WPB, NU_D, 2>(P, stream);
+    return warp_op<VARIANT, WPB, NU_D, 4>(P, stream);
 }
 
 template <int VARIANT, int WPB>
@@ -427,13 +408,18 @@ static int warp_op_d(int nud, int nup, const SweepParams *P, cudaStream_t stream
 {
     if (nud == 0) return warp_op_p<VARIANT, WPB, 0>(nup, P, stream);
     if (nud == 1) return warp_op_p<VARIANT, WPB, 1>(nup, P, stream);
-    return warp_op_p<VARIANT, WPB, 4>(nup, P, stream);
+    return warp_op_p<VARIANT, WPB, 6>(nup, P, stream);
 }
 
 static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams *P, cudaStream_t stream)
 {
-    if (variant == 0) return wpb == 7 ? warp_op_d<0, 7>(nud, nup, P, stream) : warp_op_d<0, 1>(nud, nup, P, stream);
-    return wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream) : warp_op_d<1, 1>(nud, nup, P, stream);
+    if (variant == 0)
+        return wpb == 14  ? warp_op_d<0, 14>(nud, nup, P, stream)
+               : wpb == 7 ? warp_op_d<0, 7>(nud, nup, P, stream)
+                          : warp_op_d<0, 1>(nud, nup, P, stream);
+    return wpb == 14  ? warp_op_d<1, 14>(nud, nup, P, stream)
+           : wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream)
+                      : warp_op_d<1, 1>(nud, nup, P, stream);
 }
 
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
@@ -443,7 +429,7 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
 
 int configure_warp_kernels()
 {
-    const int nuds[3] = {0, 1, 4}, nups[3] = {0, 1, 2}, wpbs[2] = {7, 1};
+    const int nuds[3] = {0, 1, 6}, nups[3] = {0, 1, 4}, wpbs[3] = {14, 7, 1};
     for (int variant = 0; variant < 2; ++variant)
         for (int wpb : wpbs)
             for (int nud : nuds)
