@@ -33,6 +33,9 @@ import numpy as np
 import workloads as wl
 
 SWEEPS_PER_STEP = 10
+# dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch from the committed `ncu --set full` capture
+# (profiles/), per config; None where no capture exists.
+NCU_TRAFFIC_BYTES = {"cfg4": 2.090e9}   # profiles/r1b_sweep_kernel_full.md
 METRIC = "replica_site_updates_per_sec"
 UNIT = "replica-site updates/s"
 
@@ -54,17 +57,24 @@ def nplanes_of(q: float) -> int:
     return 32 - ((T & -T).bit_length() - 1)
 
 
-INSTR_PER_BLOCK_LAZY = 51.0   # 20 IMAD.WIDE + 20 LOP3 + counter set-up + MSB-first compare of 2 planes
-INSTR_PER_BLOCK_EAGER = 46.0
+# Per-block and fixed thread-instruction counts of the sweep kernel's own SASS (sweep_warp.cu, nvcc 12.9):
+# one strength-reduced Philox-4x32-10 block = 16 IMAD.WIDE.U32 + 18 LOP3; MSB-first compare of its two planes
+# = 8 LOP3 (2 per plane per 32-lane half in the minimal masked form; the kernel's branch-free form uses 10);
+# per attempt: 2 IMAD.WIDE (slot constants) + 1 IMAD.HI (position) and ~40 logic/address ops (rule 22,
+# position/seam/address 12, tail masks 6; TCPD +6).
+WIDE_PER_BLOCK, ALU_PER_BLOCK = 16.0, 18.0 + 8.0
+WIDE_FIXED = 3.0
 
 
 def algorithmic_instr_per_attempt_word(cfg: wl.Config) -> dict:
-    F = 90.0 if cfg.variant == wl.PCPD else 100.0
+    alu_fixed = 40.0 if cfg.variant == wl.PCPD else 46.0
     npd, npp = nplanes_of(cfg.d), nplanes_of(cfg.p)
-    lazy_blocks = blocks_needed_generic(npd) + blocks_needed_generic(npp)
-    eager_blocks = (npd + 1) // 2 + (npp + 1) // 2
-    return dict(lazy=F + INSTR_PER_BLOCK_LAZY * lazy_blocks, eager=F + INSTR_PER_BLOCK_EAGER * eager_blocks,
-                lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=F)
+    lazy_blocks = 1.0 + blocks_needed_generic(npd) + blocks_needed_generic(npp)   # + the MISC block
+    eager_blocks = 1.0 + (npd + 1) // 2 + (npp + 1) // 2
+    per_block = WIDE_PER_BLOCK + ALU_PER_BLOCK
+    fixed = WIDE_FIXED + alu_fixed
+    return dict(lazy=fixed + per_block * lazy_blocks, eager=fixed + per_block * eager_blocks,
+                lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=fixed, per_block=per_block)
 
 
 def load_peaks() -> dict:
@@ -286,22 +296,32 @@ def ours_arm(args, cfg: wl.Config) -> None:
     if rank == 0:
         alg = algorithmic_instr_per_attempt_word(cfg)
         attempt_words = float(cfg.L) * cfg.W                      # per sweep launch
-        issue_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6        # thread-instr/s, 4 schedulers x 32 lanes per SM
+        # INT roofline.  Nominal issue peak = 4 schedulers x 32 lanes per SM per clock.  The
+        # kernel's instruction mix (IMAD.WIDE.U32 + ALU-pipe logic) cannot reach it: measured by microbenchmark 5
+        # (one wide multiply + three LOP3 per step, run live here) every instruction of that mix costs 2 issue
+        # cycles per scheduler, i.e. the mix peaks at ~64 lanes/clk/SM.  `peak` is that measured rate.
+        nominal_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6
+        mix_peak = pk.microbench(5, 4000)                          # thread-instr/s, measured on this GPU now
         achieved = alg["lazy"] * attempt_words / (sweep_ms * 1e-3)
         hbm_bytes = 2.0 * cfg.lattice_bytes
-        roof = dict(bound="alu", achieved=achieved / 1e12, peak=issue_peak / 1e12, unit="Tinstr/s",
-                    frac=achieved / issue_peak, traffic=None,
-                    kernel="sweep_kernel", launch_ms=sweep_ms,
+        roof = dict(bound="alu", achieved=achieved / 1e12, peak=mix_peak / 1e12, unit="Tinstr/s",
+                    frac=achieved / mix_peak, traffic=NCU_TRAFFIC_BYTES.get(cfg.name),
+                    kernel="sweep_warp_kernel", launch_ms=sweep_ms,
                     instr_per_attempt_word=alg["lazy"], lazy_blocks=alg["lazy_blocks"],
-                    frac_eager=alg["eager"] * attempt_words / (sweep_ms * 1e-3) / issue_peak,
-                    peak_source=f"148 SMs x 128 thread-instr/clk x {peaks['sm_max_mhz']:.0f} MHz (guide unit counts)",
+                    frac_eager=alg["eager"] * attempt_words / (sweep_ms * 1e-3) / mix_peak,
+                    frac_of_nominal_issue=achieved / nominal_peak,
+                    peak_source="measured live: pcpd_microbench(5), IMAD.WIDE.U32 + 3 LOP3 mix on all SMs "
+                                f"({mix_peak / 148 / (peaks['sm_max_mhz'] * 1e6):.1f} lanes/clk/SM); nominal issue peak "
+                                f"148 SMs x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz = {nominal_peak / 1e12:.1f} Tinstr/s",
                     hbm=dict(achieved=hbm_bytes / (sweep_ms * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
                              frac=hbm_bytes / (sweep_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], peak_source=peaks["source"]))
         cores = max(1, min(os.cpu_count() or 1, cfg.W, 16))
         L_sample = min(cfg.L, 1 << 17)
-        cpu_rate, cpu_dt = oracle_sample_rate(cfg, L_sample, cores, 1)
+        _, dt1 = oracle_sample_rate(cfg, L_sample, cores, 1)         # calibration sweep
+        n_sw = int(max(1, min(200, round(15.0 / max(dt1, 1e-3)))))   # about 15 s of CPU work
+        cpu_rate, cpu_dt = oracle_sample_rate(cfg, L_sample, cores, n_sw)
         sample = (f"{cfg.name} parameters on a ring of L = {L_sample} sites, word columns 0..{cores - 1} of {cfg.W}, "
-                  f"1 sweep, one thread per column ({cpu_dt:.1f} s)")
+                  f"{n_sw} sweeps, one thread per column ({cpu_dt:.1f} s)")
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                     ms_per_step=t_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                     dtype="u64", data="synthetic",

@@ -42,6 +42,28 @@ int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_off
 }
 
 // --------------------------------------------------------------- permute ---
+// canonical [L][W] <-> physical column-major [W][L]: a tiled transpose through shared memory
+// (32 x 32 words, padded), both sides coalesced.  General word-blocked layouts (Wb > 1) take the
+// simple gather below; only get/set_lattice use either, never pcpd_run.
+__global__ void __launch_bounds__(256) transpose_kernel(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst,
+                                                        uint32_t rows, uint32_t cols)
+{
+    // src is rows x cols row-major, dst is cols x rows row-major
+    __shared__ uint64_t t[32][33];
+    const uint32_t tiles_c = (cols + 31) / 32;
+    const uint32_t c0 = (blockIdx.x % tiles_c) * 32, r0 = (blockIdx.x / tiles_c) * 32;
+    const uint32_t tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (uint32_t j = ty; j < 32; j += 8) {
+        const uint32_t r = r0 + j, c = c0 + tx;
+        if (r < rows && c < cols) t[j][tx] = src[(size_t)r * cols + c];
+    }
+    __syncthreads();
+    for (uint32_t j = ty; j < 32; j += 8) {
+        const uint32_t c = c0 + j, r = r0 + tx;
+        if (r < rows && c < cols) dst[(size_t)c * rows + r] = t[tx][j];
+    }
+}
+
 __global__ void permute_kernel(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst, uint32_t L, uint32_t W,
                                uint32_t Wb, int to_physical)
 {
@@ -57,6 +79,15 @@ __global__ void permute_kernel(const uint64_t *__restrict__ src, uint64_t *__res
 int launch_permute(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int Wb, int to_physical,
                    cudaStream_t stream)
 {
+    if (Wb == 1) {
+        // to_physical: src = canonical L x W; else src = physical W x L
+        const uint32_t rows = to_physical ? L : W, cols = to_physical ? W : L;
+        const uint64_t tiles = (uint64_t)((cols + 31) / 32) * ((rows + 31) / 32);
+        if (tiles < (1ull << 31)) {
+            transpose_kernel<<<(uint32_t)tiles, 256, 0, stream>>>(src, dst, rows, cols);
+            return 1;
+        }
+    }
     const size_t total = (size_t)L * W;
     int blocks = (int)((total + 255) / 256);
     if (blocks > 148 * 16) blocks = 148 * 16;
