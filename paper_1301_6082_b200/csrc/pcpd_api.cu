@@ -200,6 +200,15 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         P.tdm[k] = ((P.thd.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
         P.tpm[k] = ((P.thp.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
     }
+    auto tbit = [](uint32_t T32, int k) -> int32_t { return (k < 0 || k > 31) ? 0 : (int32_t)((T32 >> (31 - k)) & 1u); };
+    for (int k = 0; k < 34; ++k) {
+        P.sd[k] = tbit(P.thd.T32, k) - tbit(P.thd.T32, k - 1);
+        P.sp[k] = tbit(P.thp.T32, k) - tbit(P.thp.T32, k - 1);
+    }
+    for (int M = 0; M < 18; ++M) {
+        P.cld[M] = -tbit(P.thd.T32, 2 * M - 1);
+        P.clp[M] = -tbit(P.thp.T32, 2 * M - 1);
+    }
     g_err[0] = 0;
     return h;
 }

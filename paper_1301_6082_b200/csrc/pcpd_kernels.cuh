@@ -30,6 +30,11 @@ struct SweepParams {
     // T's bit for plane k (bit 31-k) as an all-ones / all-zeros 32-lane mask, precomputed on the
     // host so that the kernels read them as constant-bank operands (C3)
     uint32_t tdm[32], tpm[32];
+    // Signed-sum form of the compare: with und_k the lanes still equal to T
+    // before plane k (nested sets), lt = sum_k s_k * und_k with s_k = tb_k - tb_(k-1) in {-1,0,+1}
+    // (tb_(-1) = tb_32 = 0); stopping after M blocks closes the sum with cl[M] = -tb_(2M-1).
+    int32_t sd[34], sp[34];
+    int32_t cld[18], clp[18];
 };
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.

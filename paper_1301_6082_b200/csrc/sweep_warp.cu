@@ -165,6 +165,27 @@ __device__ __forceinline__ void cmp_block(Mask2 &lt, Mask2 &und, const U4 &blk, 
     cmp2h(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1);
 }
 
+// Signed-sum form of the same compare.  und_k (lanes still equal to T before plane k) are nested
+// sets, and lt = OR_k (und_k - und_(k+1)) over the planes where T's bit is 1 = sum_k s_k * und_k with
+// s_k = tb_k - tb_(k-1) in {-1, 0, +1}: the lt accumulation becomes one 32-bit IMAD per plane and half
+// (FMA pipe, which has slack) and only the und chain (one LOP3 per plane and half) stays on the ALU
+// pipe, the binding one.  The caller closes the sum with -tb_last * und when it stops.
+__device__ __forceinline__ void cmp2h_sum(uint32_t &lt, uint32_t &und, uint32_t p0, uint32_t p1, uint32_t tb0,
+                                          uint32_t tb1, int32_t s0, int32_t s1)
+{
+    lt += und * (uint32_t)s0;
+    const uint32_t u1 = und & ~(p0 ^ tb0);
+    lt += u1 * (uint32_t)s1;
+    und = u1 & ~(p1 ^ tb1);
+}
+
+__device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &blk, uint32_t tb0, uint32_t tb1,
+                                              int32_t s0, int32_t s1)
+{
+    cmp2h_sum(lt.lo, und.lo, blk.x0, blk.x2, tb0, tb1, s0, s1);
+    cmp2h_sum(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1, s0, s1);
+}
+
 // T's bit for plane k (bit 31-k) as a 32-lane mask.
 __device__ __forceinline__ uint32_t tmask(uint32_t T32, uint32_t k)
 {
@@ -284,19 +305,26 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
 #pragma unroll
-            for (int m = 0; m < NU_D; ++m) cmp_block(dlt, dund, dblk[m], P.tdm[2 * m], P.tdm[2 * m + 1]);
+            for (int m = 0; m < NU_D; ++m)
+                cmp_block_sum(dlt, dund, dblk[m], P.tdm[2 * m], P.tdm[2 * m + 1], P.sd[2 * m], P.sd[2 * m + 1]);
 #pragma unroll
-            for (int m = 0; m < NU_P; ++m) cmp_block(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1]);
+            for (int m = 0; m < NU_P; ++m)
+                cmp_block_sum(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m], P.sp[2 * m + 1]);
             {
                 const uint64_t rel = sb | sc;
                 dund.lo &= (uint32_t)rel;
                 dund.hi &= (uint32_t)(rel >> 32);
                 uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top (0 past the last plane)
-                for (uint32_t m = NU_D; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
+                uint32_t m = NU_D;
+                for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, P.rk);
-                    cmp_block(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
+                    cmp_block_sum(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31),
+                                  P.sd[2 * m], P.sd[2 * m + 1]);
                     Tsh <<= 2;
                 }
+                // close the sum: lanes still equal to T after the last plane looked at are not < T
+                dlt.lo += dund.lo * (uint32_t)P.cld[m];
+                dlt.hi += dund.hi * (uint32_t)P.cld[m];
             }
             const uint64_t Dm = P.thd.all ? ~0ull : m64(dlt);
             uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
@@ -305,11 +333,15 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 pund.lo &= (uint32_t)react;
                 pund.hi &= (uint32_t)(react >> 32);
                 uint32_t Tsh = Tp << (2 * NU_P);
-                for (uint32_t m = NU_P; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
+                uint32_t m = NU_P;
+                for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, P.rk);
-                    cmp_block(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31));
+                    cmp_block_sum(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31),
+                                  P.sp[2 * m], P.sp[2 * m + 1]);
                     Tsh <<= 2;
                 }
+                plt.lo += pund.lo * (uint32_t)P.clp[m];
+                plt.hi += pund.hi * (uint32_t)P.clp[m];
             }
             const uint64_t Pm = P.thp.all ? ~0ull : m64(plt);
 
