@@ -179,7 +179,7 @@ static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
 
 int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream)
 {
-    if (Wb == 1 && sweep_warp_supported(P.Ts, P.D)) return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts), stream);
+    if (Wb == 1 && sweep_warp_supported(P.Ts, P.D)) return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream);
     if (variant == 0) {
         if (Wb == 4) return launch_sweep_t<0, 4>(P, stream);
         if (Wb == 2) return launch_sweep_t<0, 2>(P, stream);

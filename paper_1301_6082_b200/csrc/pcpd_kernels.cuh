@@ -41,7 +41,7 @@ struct SweepParams {
 int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream);
 // warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
-int sweep_warp_wpb(uint32_t Ts);
+int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream);
 int configure_warp_kernels();
 int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,

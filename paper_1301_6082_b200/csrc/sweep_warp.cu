@@ -402,17 +402,24 @@ bool sweep_warp_supported(uint32_t Ts, uint32_t D)
 }
 
 // warps per block: as many as fit 227 KB / SM in at most a few blocks
-int sweep_warp_wpb(uint32_t Ts)
+int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks)
 {
+    if (ntasks < 148ull * 14) return 1;    // small problem: one warp per block so that the warps spread over all SMs
     const size_t per = warp_smem_bytes(Ts, 1);
     if (14 * per <= 113 * 1024) return 14; // 2 blocks x 14 warps per SM at T_s = 1024 (2 x (114912 + 1024) B)
     if (7 * per <= 113 * 1024) return 7;   // 2 blocks x 7 warps per SM at T_s = 2048 (2 x (114800 + 1024) B)
     return 1;
 }
 
-// prefix lengths for a threshold with nblk blocks
-static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 6 ? 1 : 6; }
-static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < 4 ? 1 : 4; }
+// prefix lengths for a threshold with nblk blocks (tuned on B200 at cfg4)
+#ifndef PCPD_NUD_BIG
+#define PCPD_NUD_BIG 5
+#endif
+#ifndef PCPD_NUP_BIG
+#define PCPD_NUP_BIG 4
+#endif
+static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUD_BIG ? 1 : PCPD_NUD_BIG; }
+static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUP_BIG ? 1 : PCPD_NUP_BIG; }
 
 template <int VARIANT, int WPB, int NU_D, int NU_P>
 static int warp_op(const SweepParams *P, cudaStream_t stream)
@@ -432,7 +439,7 @@ static int warp_op_p(int nup, const SweepParams *P, cudaStream_t stream)
 {
     if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0>(P, stream);
     if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1>(P, stream);
-    return warp_op<VARIANT, WPB, NU_D, 4>(P, stream);
+    return warp_op<VARIANT, WPB, NU_D, PCPD_NUP_BIG>(P, stream);
 }
 
 template <int VARIANT, int WPB>
@@ -440,7 +447,7 @@ static int warp_op_d(int nud, int nup, const SweepParams *P, cudaStream_t stream
 {
     if (nud == 0) return warp_op_p<VARIANT, WPB, 0>(nup, P, stream);
     if (nud == 1) return warp_op_p<VARIANT, WPB, 1>(nup, P, stream);
-    return warp_op_p<VARIANT, WPB, 6>(nup, P, stream);
+    return warp_op_p<VARIANT, WPB, PCPD_NUD_BIG>(nup, P, stream);
 }
 
 static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams *P, cudaStream_t stream)
@@ -461,7 +468,7 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
 
 int configure_warp_kernels()
 {
-    const int nuds[3] = {0, 1, 6}, nups[3] = {0, 1, 4}, wpbs[3] = {14, 7, 1};
+    const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[3] = {0, 1, PCPD_NUP_BIG}, wpbs[3] = {14, 7, 1};
     for (int variant = 0; variant < 2; ++variant)
         for (int wpb : wpbs)
             for (int nud : nuds)
