@@ -44,6 +44,8 @@ def lib() -> C.CDLL:
         L.oracle_threshold.restype = C.c_uint64
         L.oracle_lane_uniforms.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, u32p]
         L.oracle_lane_uniforms.restype = None
+        L.oracle_paper_pmask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
+        L.oracle_paper_pmask.restype = None
         L.oracle_bernoulli_mask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
         L.oracle_bernoulli_mask.restype = None
         L.oracle_single_attempt.argtypes = [C.c_int, C.c_uint32, u8p, C.c_uint32, C.c_int, C.c_int, C.c_int]
@@ -110,6 +112,16 @@ def bernoulli_mask(seed, slot, sweep, word, stream, T) -> np.ndarray:
     m = np.zeros(64, dtype=np.uint8)
     lib().oracle_bernoulli_mask(seed, slot, sweep, word, stream, T, _p(m, C.c_uint8))
     return m
+
+
+def paper_pmask(seed, slot, sweep, word, T4p) -> np.ndarray:
+    """The paper's partially correlated annihilation mask (oracle_paper_pmask)."""
+    m = np.zeros(64, dtype=np.uint8)
+    lib().oracle_paper_pmask(seed, slot, sweep, word, T4p, _p(m, C.c_uint8))
+    return m
+
+
+PMASK_PAPER = 0x100  # variant flag: the paper's own annihilation mask (needs p < 1/4)
 
 
 def single_attempt(variant, q, i, Dm, Pm, Fm) -> np.ndarray:

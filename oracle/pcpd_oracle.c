@@ -22,6 +22,10 @@
  *                                 isolated particles, master-equation enumeration
  *                                 of eq. (1) on rings L<=6
  *   oracle_literal_*          P4  exact E[rho] from the master equation
+ *   oracle_paper_pmask        P9  the paper's own annihilation mask (Alg. 2 l.12-13):
+ *                                 lane probability p, word-wide gate 4p, lanes
+ *                                 independent 1/4-bits given the gate, pair
+ *                                 probability p/4; P5 bias check vs literal Alg. 1
  *   oracle_run (schedule SD2) P5  vs literal Alg. 1 (statistical), P6 exact toy
  *                                 operator, P7 run splitting / loop order /
  *                                 word subsets
@@ -147,6 +151,27 @@ static void bernoulli_lanes(uint64_t seed, uint32_t slot, uint32_t sweep, uint32
     if (need) *need = planes_needed(U, T);
 }
 
+/* C4' - the paper's own annihilation mask (Alg. 2 lines 12-13; section 4.3,
+ * PAPER.md:157-161), next-row f2 of SURVEY.md 8(f).  "aMask := RNG() and RNG()": two independent
+ * raw random words give every lane an independent bit that is 1 w.p. 1/4 - here the two planes
+ * `lo`, `hi` of ANNI block 0; "(RNG() < 4p) ? 1 : 0 ... gives either 1 or 0 equally for all N_r
+ * bits": ONE uniform per attempt-word, shared by its 64 lanes - here x3 of the MISC
+ * block (unused by C4), compared as a 32-bit integer with T4p = floor(4p * 2^32).  Lane j of the
+ * mask = lo_j and hi_j and [x3 < T4p]: probability (1/4)(T4p/2^32) ~ p per lane, lanes partially
+ * correlated.  Requires p < 1/4. */
+void oracle_paper_pmask(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
+                        uint64_t T4p, uint8_t mask[64])
+{
+    uint32_t a[4], misc[4];
+    block(seed, slot, sweep, word, STREAM_ANNI, 0, a);
+    block(seed, slot, sweep, word, STREAM_MISC, 0, misc);
+    uint64_t lo = (uint64_t)a[0] | ((uint64_t)a[1] << 32);
+    uint64_t hi = (uint64_t)a[2] | ((uint64_t)a[3] << 32);
+    int gate = ((uint64_t)misc[3] < T4p) ? 1 : 0;
+    for (int j = 0; j < 64; ++j)
+        mask[j] = (uint8_t)(((lo >> j) & 1u) && ((hi >> j) & 1u) && gate);
+}
+
 void oracle_bernoulli_mask(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
                            uint32_t stream, uint64_t T, uint8_t mask[64])
 {
@@ -201,8 +226,9 @@ void oracle_single_attempt(int variant, uint32_t L, uint8_t *q, uint32_t i,
 /* --------------------------------------------------------------- handle --- */
 typedef struct oracle_t {
     uint32_t L, Ts, D, A;
-    int variant;
-    uint64_t Td, Tp;
+    int variant;               /* 0 PCPD, 1 TCPD */
+    int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
+    uint64_t Td, Tp, T4p;
     uint64_t seed;
     uint32_t sweep;            /* C7: state = lattice + sweep counter */
     uint32_t nwords;           /* word columns simulated (subset of the full run) */
@@ -221,7 +247,12 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
                         uint32_t Ts, uint32_t D, uint32_t A,
                         uint32_t nwords, const uint32_t *words)
 {
+    /* variant = base | ORACLE_PMASK_PAPER (0x100): base 0 PCPD / 1 TCPD; the flag selects the
+     * paper's partially correlated annihilation mask, which needs p < 1/4. */
+    int pmask_paper = (variant & 0x100) ? 1 : 0;
+    variant &= ~0x100;
     if (variant != 0 && variant != 1) return NULL;
+    if (pmask_paper && !(p < 0.25)) return NULL;
     uint32_t Rr = variant == 0 ? 2u : 3u;
     if (L == 0 || L >= ((uint64_t)1 << 32) || nwords == 0) return NULL;
     if (Ts > L) Ts = (uint32_t)L;
@@ -233,6 +264,8 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     oracle_t *o = (oracle_t *)calloc(1, sizeof *o);
     if (!o) return NULL;
     o->L = (uint32_t)L; o->Ts = Ts; o->D = D; o->A = A; o->variant = variant;
+    o->pmask_paper = pmask_paper;
+    o->T4p = pmask_paper ? oracle_threshold(4.0 * p) : 0;   /* floor(4p * 2^32) < 2^32 since p < 1/4 */
     o->Td = Td; o->Tp = Tp; o->seed = seed; o->sweep = 0; o->nwords = nwords;
     o->words = (uint32_t *)malloc(sizeof(uint32_t) * nwords);
     o->q = (uint8_t *)calloc((size_t)nwords * 64 * (size_t)L, 1);
@@ -319,7 +352,8 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
     uint8_t Dm[64], Pm[64];
     int needD = 0, needP = 0;
     bernoulli_lanes(o->seed, g, t, w, STREAM_DIFF, o->Td, Dm, &needD);
-    bernoulli_lanes(o->seed, g, t, w, STREAM_ANNI, o->Tp, Pm, &needP);
+    if (o->pmask_paper) { oracle_paper_pmask(o->seed, g, t, w, o->T4p, Pm); needP = 2; }
+    else bernoulli_lanes(o->seed, g, t, w, STREAM_ANNI, o->Tp, Pm, &needP);
     o->n_attempt_words += 1;
     o->planes_needed_D += (uint64_t)needD; o->planes_needed_P += (uint64_t)needP;
     o->blocks_needed_D += (uint64_t)((needD + 1) / 2);

@@ -8,16 +8,14 @@
 // in one warp, sub-steps need __syncwarp() only - no block barrier anywhere in
 // the sweep.
 //
-// Per sub-step the A attempts of a lane are processed in batches of NB:
-//   phase A (state-independent, so batched over the NB attempts for ILP):
-//           MISC block -> position x, fission-side mask Fm;
-//           DIFF planes -> Dm on all 64 lanes, NU_D blocks unconditionally,
-//           then lazily while any lane of the warp is undecided;
-//   phase B (sequential in a): load the footprint, react = pair & ~Dm, ANNI
-//           planes lazily on the react lanes only, bitwise rule, store.
-// Philox rounds 1-3 are strength-reduced: the products that depend only on
-// (w, t) or only on the slot are computed once per warp / once per attempt,
-// leaving 16 IMAD.WIDE.U32 per block instead of 20.
+// Per attempt a lane issues, as one basic block, 1 + NU_D + NU_P independent Philox chains
+// (MISC block, the first NU_D DIFF blocks, the first NU_P ANNI blocks: none depends on the lattice
+// state) written round-major so that ptxas interleaves them; the planes are compared MSB-first
+// against T's bits on all 64 lanes in the signed-sum form (und chain on the ALU pipe, lt
+// accumulation as IMADs on the FMA pipe); the lazy tails then run as warp-uniform loops only while
+// some lane whose outcome can matter is undecided (DIFF: x or x+1 occupied; ANNI: reacting lanes).
+// Philox rounds 1-3 are strength-reduced: the products that depend only on (w, t) or only on the
+// slot are computed once per warp / once per attempt, leaving 16 IMAD.WIDE.U32 per block, not 20.
 //
 // Citations: update rule = Alg. 1 PAPER.md:45-70 in the bitwise form of Alg. 2
 // PAPER.md:126-151 (typos fixed per DESIGN.md readings G5/G6); schedule SD2 and
@@ -195,9 +193,9 @@ __device__ __forceinline__ uint32_t tmask(uint32_t T32, uint32_t k)
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
-// parameters so that the unconditional part has no branch at all).  A warp needs DIFF block 3
-// w.p. > 0.999 when the threshold has >= 8 planes, so NU_D = 4 there; ANNI matters only on the
-// reacting lanes (a few per word), so NU_P = 2.  Thresholds with fewer planes get fewer blocks.
+// parameters so that the unconditional part has no branch at all): 5 and 4 for thresholds with that
+// many blocks (tuned on B200: a warp pays the maximum over its 32 lanes, so nearly every attempt
+// needs that many anyway), 1 for thresholds with few planes (d = 1/2 has one), 0 for T = 0 or 2^32.
 template <int VARIANT, int WPB, int NU_D, int NU_P>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {

@@ -329,3 +329,52 @@ def test_create_rejects_invalid():
         oracle.Oracle(128, 64, 1.5, 0.1, 1, 0)
     with pytest.raises(ValueError):
         oracle.Oracle(128, 64, 0.5, 0.1, 1, 0, Ts=8, D=8, A=2).__class__(128, 64, 0.5, 0.1, 1, 1, Ts=8, D=8, A=2)  # TCPD needs D>=9
+
+
+# ------------------------------------------------------------------ P9 ----
+# The paper's own annihilation mask (next-row f2; Alg. 2 lines 12-13 PAPER.md:141-142,
+# section 4.3): "RNG() and RNG()" = an independent 1/4-bit per lane,
+# ANDed with ONE word-wide draw that is 1 w.p. 4p.  Pinned to what the paper fixes: the
+# per-lane probability is p; given the word-wide draw the lanes are independent 1/4-bits;
+# two lanes are both set w.p. (1/16) 4p = p/4 (partially correlated);
+# the word is empty whenever the word-wide draw fails.
+def test_P9_paper_pmask_probabilities():
+    p = 0.12
+    T4p = oracle.threshold(4 * p)
+    assert T4p == int(np.floor(4 * p * 2.0 ** 32))
+    n = 40000
+    masks = np.array([oracle.paper_pmask(11, s, 3, s % 7, T4p) for s in range(n)], dtype=np.float64)  # [n, 64]
+    gate = masks.any(axis=1)
+    # per-lane probability p: words are the independent samples (lanes of a word share the draw)
+    per_word = masks.mean(axis=1)
+    se = per_word.std(ddof=1) / n ** 0.5
+    assert abs(per_word.mean() - p) < 4 * se, (per_word.mean(), p, se)
+    # P(word-wide draw = 1) = 4p, up to the words whose 64 quarter-bits are all 0 (prob. (3/4)^64 ~ 1e-8)
+    assert abs(gate.mean() - 4 * p) < 4 * (4 * p * (1 - 4 * p) / n) ** 0.5
+    # given the draw, lanes are independent Bernoulli(1/4)
+    g = masks[gate]
+    assert abs(g.mean() - 0.25) < 4 * (0.25 * 0.75 / g.size) ** 0.5
+    c = np.corrcoef(g[:, :8].T)
+    assert np.all(np.abs(c - np.eye(8)) < 5 / len(g) ** 0.5)
+    # two lanes both set: p/4, not p^2 (independent) and not p (fully correlated)
+    both = (masks[:, 0] * masks[:, 1]).mean()
+    assert abs(both - p / 4) < 4 * (p / 4 / n) ** 0.5
+    # threshold edge cases: T4p = 0 never annihilates
+    assert not any(oracle.paper_pmask(11, s, 3, 0, 0).any() for s in range(200))
+
+
+def test_P9_paper_pmask_mode_in_run():
+    """The run uses exactly that mask: a full lattice with d = 0 (no diffusion) loses particles
+    only in words whose word-wide draw fired, and p >= 1/4 is rejected."""
+    with pytest.raises(ValueError):
+        oracle.Oracle(128, 64, 0.5, 0.25, 1, oracle.PMASK_PAPER, Ts=64, D=16, A=4)
+    kw = dict(L=64, n_replicas=64, d=0.0, p=0.2, seed=5, Ts=64, D=16, A=16)
+    a = oracle.Oracle(variant=oracle.PMASK_PAPER, **kw)
+    b = oracle.Oracle(variant=0, **kw)
+    a.init(wl.INIT_FULL)
+    b.init(wl.INIT_FULL)
+    a.run(1)
+    b.run(1)
+    # same positions and fission bits, different annihilation masks -> different states
+    assert not np.array_equal(a.get_words(), b.get_words())
+    assert a.counts().min() < 64  # something was annihilated at p = 0.2

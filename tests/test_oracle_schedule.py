@@ -158,7 +158,7 @@ def _sd2_vs_literal(variant, L, R, d, p, times, sch, seed=7):
         prev = t
         sd2.append(o.counts().astype(np.float64).reshape(W, 64).mean(axis=1) / L)  # per word
     sd2 = np.array(sd2)                                                       # [n_t, W]
-    lit, _ = oracle.literal_run(variant, L, R, d, p, seed + 1000, np.ones((R, L), np.uint8), times)
+    lit, _ = oracle.literal_run(variant & 0xff, L, R, d, p, seed + 1000, np.ones((R, L), np.uint8), times)
     lit = lit.astype(np.float64) / L                                          # [n_t, R]
     m_s, e_s = sd2.mean(axis=1), sd2.std(axis=1, ddof=1) / W ** 0.5
     m_l, e_l = lit.mean(axis=1), lit.std(axis=1, ddof=1) / R ** 0.5
@@ -183,3 +183,15 @@ def test_P5_tcpd_sd2_matches_literal():
     z, rel, _, _ = _sd2_vs_literal(wl.TCPD, 512, 1024, 0.5, 0.05, times, dict(Ts=2048, D=64, A=4))
     print("P5 tcpd z =", np.round(z, 2), "rel =", np.round(rel, 4))
     assert np.all(np.abs(z) < 4.0), (z, rel)
+
+
+@pytest.mark.slow
+def test_P5_paper_pmask_sd2_matches_literal():
+    """The paper's partially correlated annihilation mask must not bias rho(t):
+    the paper's own check - compare with the literal Algorithm 1, whose draws
+    are independent per replica.  Words are the independent samples (reading G12)."""
+    times = [1, 2, 4, 8, 16, 32, 64]
+    z, rel, _, _ = _sd2_vs_literal(wl.PCPD | oracle.PMASK_PAPER, 512, 4096, 0.5, 0.15, times, dict(Ts=2048, D=64, A=4))
+    print("P5 paper-pmask z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)
+    assert np.all(np.abs(rel) < 0.02), rel
