@@ -53,6 +53,15 @@ enum pcpd_status {
 };
 
 enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1 };
+/* Flag to OR into `variant`: use the PAPER's OWN annihilation mask instead of independent
+ * per-lane Bernoulli(p) bits (Alg. 2 lines 12-13; section 4.3):
+ * lane j of Pm = a0_j & a1_j & [u < 4p], a0/a1 = the two 64-lane planes of ANNI block 0 (an
+ * independent 1/4-bit per lane), u = x3 of the MISC block, ONE draw per attempt-word shared by
+ * its 64 lanes, compared as a 32-bit integer with floor(4p * 2^32).  Each lane is 1 w.p. p but
+ * lanes of a word are partially correlated.  Requires p < 1/4 (else PCPD_ERR_ARG).
+ * Costs 3 Philox blocks per attempt-word when d is a short dyadic (d = 1/2, 1/4, 3/4: the
+ * paper's AND/OR recipe for d, is what C3 reduces to for such d). */
+#define PCPD_VARIANT_PMASK_PAPER 0x100
 enum pcpd_init_mode { PCPD_INIT_FULL = 0, PCPD_INIT_BERNOULLI = 1, PCPD_INIT_EMPTY = 2 };
 
 /* Default schedule constants of SD2 (C5). */

@@ -99,6 +99,8 @@ int pcpd_set_allocator(pcpd_alloc_fn alloc, pcpd_free_fn release)
 pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant, uint32_t Ts,
                        uint32_t D, uint32_t A, uint64_t word_offset)
 {
+    const int pmask_paper = (variant & PCPD_VARIANT_PMASK_PAPER) ? 1 : 0;
+    variant &= ~PCPD_VARIANT_PMASK_PAPER;
     if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD) {
         fail(PCPD_ERR_ARG, "unknown variant %d", variant);
         return nullptr;
@@ -111,6 +113,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     const uint64_t W = n_replicas / 64;
     if (!(d >= 0.0 && d <= 1.0) || !(p >= 0.0 && p <= 1.0)) {
         fail(PCPD_ERR_ARG, "d and p must lie in [0,1]");
+        return nullptr;
+    }
+    if (pmask_paper && !(p < 0.25)) {
+        fail(PCPD_ERR_ARG, "the paper's annihilation mask needs p < 1/4");
         return nullptr;
     }
     if (L == 0 || L >= (1ull << 32) || word_offset + W >= (1ull << 32)) {
@@ -141,6 +147,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     // Physical layout: column-major [W][L] (word-group width Wb = 1): a tile column is one
     // contiguous run of T_s words, which is what the warp-per-(tile, column) sweep kernel loads.
     const int Wb = 1;
+    if (pmask_paper && !sweep_warp_supported(Ts, D)) {
+        fail(PCPD_ERR_ARG, "the paper's annihilation mask needs at most 32 domains per tile (T_s / D <= 32)");
+        return nullptr;
+    }
     if (!sweep_warp_supported(Ts, D) && (sweep_smem_bytes(Ts, Wb) > 200 * 1024 || (uint64_t)(Ts / D) > 1024)) {
         fail(PCPD_ERR_ARG, "schedule: tile of %u sites does not fit one thread block", Ts);
         return nullptr;
@@ -196,6 +206,8 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     P.thd = make_threshold(h->Td);
     P.thp = make_threshold(h->Tp);
     P.rk = make_round_keys(seed);
+    P.pmask_paper = (uint32_t)pmask_paper;
+    P.T4p = pmask_paper ? (uint32_t)threshold_of(4.0 * p) : 0u;   // < 2^32 because p < 1/4
     for (int k = 0; k < 32; ++k) {
         P.tdm[k] = ((P.thd.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
         P.tpm[k] = ((P.thp.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;

@@ -24,7 +24,7 @@ struct SweepParams {
     uint32_t Ts, D, A, S, n;  // n = Ts / D domains per tile, S = D / A sub-steps
     uint32_t word_offset;     // global index of local column 0
     uint32_t t;               // sweep index
-    uint32_t pad;
+    uint32_t T4p;             // paper annihilation mask: floor(4p * 2^32) (pmask_paper != 0), else 0
     Threshold thd, thp;
     RoundKeys rk;
     // T's bit for plane k (bit 31-k) as an all-ones / all-zeros 32-lane mask, precomputed on the
@@ -35,6 +35,7 @@ struct SweepParams {
     // (tb_(-1) = tb_32 = 0); stopping after M blocks closes the sum with cl[M] = -tb_(2M-1).
     int32_t sd[34], sp[34];
     int32_t cld[18], clp[18];
+    uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
 };
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.

@@ -136,34 +136,15 @@ __device__ __forceinline__ void philox_blocks(const uint32_t (&c3in)[N], const P
     for (int i = 0; i < N; ++i) out[i] = U4{c0[i], c1[i], c2[i], c3[i]};
 }
 
-// MSB-first bit-sliced compare of two planes (p0 = plane 2m, p1 = plane 2m+1)
-// against T's two bits for those planes, given as all-ones / all-zeros masks
-// tb0, tb1 (C3), on one 32-lane half of the word.  Branch-free (5 LOP3), so that
-// an attempt's unconditional blocks form one basic block.
-__device__ __forceinline__ void cmp2h(uint32_t &lt, uint32_t &und, uint32_t p0, uint32_t p1, uint32_t tb0,
-                                      uint32_t tb1)
-{
-    const uint32_t u1 = und & ~(p0 ^ tb0);       // still equal to T after plane 2m
-    const uint32_t a = und & ~p0 & tb0;          // decided at plane 2m: lane bit 0, T bit 1 -> U < T
-    const uint32_t b = u1 & ~p1 & tb1;           // decided at plane 2m+1
-    und = u1 & ~(p1 ^ tb1);
-    lt |= a | b;
-}
-
 // 64-lane mask state as two 32-bit halves.
 struct Mask2 {
     uint32_t lo, hi;
 };
 __device__ __forceinline__ uint64_t m64(const Mask2 &m) { return (uint64_t)m.lo | ((uint64_t)m.hi << 32); }
 
-// block blk = planes 2m (x0 | x1 << 32) and 2m+1 (x2 | x3 << 32)
-__device__ __forceinline__ void cmp_block(Mask2 &lt, Mask2 &und, const U4 &blk, uint32_t tb0, uint32_t tb1)
-{
-    cmp2h(lt.lo, und.lo, blk.x0, blk.x2, tb0, tb1);
-    cmp2h(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1);
-}
-
-// Signed-sum form of the same compare.  und_k (lanes still equal to T before plane k) are nested
+// MSB-first bit-sliced compare of two planes (p0 = plane 2m, p1 = plane 2m+1; block blk = planes
+// x0 | x1 << 32 and x2 | x3 << 32) against T's bits tb0, tb1 given as 32-lane masks (C3), in
+// signed-sum form.  und_k (lanes still equal to T before plane k) are nested
 // sets, and lt = OR_k (und_k - und_(k+1)) over the planes where T's bit is 1 = sum_k s_k * und_k with
 // s_k = tb_k - tb_(k-1) in {-1, 0, +1}: the lt accumulation becomes one 32-bit IMAD per plane and half
 // (FMA pipe, which has slack) and only the und chain (one LOP3 per plane and half) stays on the ALU
@@ -184,19 +165,13 @@ __device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &b
     cmp2h_sum(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1, s0, s1);
 }
 
-// T's bit for plane k (bit 31-k) as a 32-lane mask.
-__device__ __forceinline__ uint32_t tmask(uint32_t T32, uint32_t k)
-{
-    return 0u - ((T32 >> (31u - k)) & 1u);
-}
-
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
 // parameters so that the unconditional part has no branch at all): 5 and 4 for thresholds with that
 // many blocks (tuned on B200: a warp pays the maximum over its 32 lanes, so nearly every attempt
 // needs that many anyway), 1 for thresholds with few planes (d = 1/2 has one), 0 for T = 0 or 2^32.
-template <int VARIANT, int WPB, int NU_D, int NU_P>
+template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
@@ -305,9 +280,11 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
 #pragma unroll
             for (int m = 0; m < NU_D; ++m)
                 cmp_block_sum(dlt, dund, dblk[m], P.tdm[2 * m], P.tdm[2 * m + 1], P.sd[2 * m], P.sd[2 * m + 1]);
+            if constexpr (PMODE == 0) {
 #pragma unroll
-            for (int m = 0; m < NU_P; ++m)
-                cmp_block_sum(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m], P.sp[2 * m + 1]);
+                for (int m = 0; m < NU_P; ++m)
+                    cmp_block_sum(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m], P.sp[2 * m + 1]);
+            }
             {
                 const uint64_t rel = sb | sc;
                 dund.lo &= (uint32_t)rel;
@@ -327,7 +304,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             const uint64_t Dm = P.thd.all ? ~0ull : m64(dlt);
             uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
             if constexpr (VARIANT == 1) react &= se;
-            {
+            if constexpr (PMODE == 0) {
                 pund.lo &= (uint32_t)react;
                 pund.hi &= (uint32_t)(react >> 32);
                 uint32_t Tsh = Tp << (2 * NU_P);
@@ -340,8 +317,15 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 }
                 plt.lo += pund.lo * (uint32_t)P.clp[m];
                 plt.hi += pund.hi * (uint32_t)P.clp[m];
+            } else {
+                // The paper's own annihilation mask (Alg. 2 lines 12-13):
+                // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
+                // word-wide draw that is 1 w.p. 4p (x3 of the MISC block against floor(4p * 2^32)).
+                const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
+                plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
+                plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
             }
-            const uint64_t Pm = P.thp.all ? ~0ull : m64(plt);
+            const uint64_t Pm = (PMODE == 0 && P.thp.all) ? ~0ull : m64(plt);
 
             // C6 / Alg. 2, branch-free over the 64 replicas.
             uint64_t nb = (Dm & sc) | (~Dm & sb);
@@ -419,15 +403,15 @@ int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks)
 static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUD_BIG ? 1 : PCPD_NUD_BIG; }
 static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUP_BIG ? 1 : PCPD_NUP_BIG; }
 
-template <int VARIANT, int WPB, int NU_D, int NU_P>
+template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE>
 static int warp_op(const SweepParams *P, cudaStream_t stream)
 {
     if (!P)  // configure
-        return (int)cudaFuncSetAttribute(sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P>,
+        return (int)cudaFuncSetAttribute(sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          WPB >= 4 ? 116 * 1024 : 226 * 1024);
     const uint32_t ntasks = (P->L / P->Ts) * P->W;
-    sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P>
+    sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE>
         <<<(ntasks + WPB - 1) / WPB, WPB * 32, warp_smem_bytes(P->Ts, WPB), stream>>>(*P);
     return 1;
 }
@@ -435,9 +419,10 @@ static int warp_op(const SweepParams *P, cudaStream_t stream)
 template <int VARIANT, int WPB, int NU_D>
 static int warp_op_p(int nup, const SweepParams *P, cudaStream_t stream)
 {
-    if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0>(P, stream);
-    if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1>(P, stream);
-    return warp_op<VARIANT, WPB, NU_D, PCPD_NUP_BIG>(P, stream);
+    if (nup == -1) return warp_op<VARIANT, WPB, NU_D, 1, 1>(P, stream);  // paper annihilation mask: ANNI block 0 only
+    if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0, 0>(P, stream);
+    if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1, 0>(P, stream);
+    return warp_op<VARIANT, WPB, NU_D, PCPD_NUP_BIG, 0>(P, stream);
 }
 
 template <int VARIANT, int WPB>
@@ -461,12 +446,13 @@ static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams
 
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
 {
-    return warp_op_any(variant, wpb, nu_d_of((P.thd.nplanes + 1) >> 1), nu_p_of((P.thp.nplanes + 1) >> 1), &P, stream);
+    const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
+    return warp_op_any(variant, wpb, nu_d_of((P.thd.nplanes + 1) >> 1), nup, &P, stream);
 }
 
 int configure_warp_kernels()
 {
-    const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[3] = {0, 1, PCPD_NUP_BIG}, wpbs[3] = {14, 7, 1};
+    const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[4] = {-1, 0, 1, PCPD_NUP_BIG}, wpbs[3] = {14, 7, 1};
     for (int variant = 0; variant < 2; ++variant)
         for (int wpb : wpbs)
             for (int nud : nuds)

@@ -111,6 +111,9 @@ SMALL = [
     (0, 1024, 128, 0.4, 0.0, 512, 64, 4, 1),         # p = 0: no annihilation
     (0, 1024, 128, 0.4, 1.0, 512, 64, 4, 1),         # p = 1: every reacting pair annihilates
     (0, 1024, 128, 2.0 ** -32, 1 - 2.0 ** -32, 512, 64, 4, 1),  # T = 1 and T = 2^32 - 1: all 32 planes matter
+    (0x100, 4096, 256, 0.75, 0.12, 2048, 64, 4, 0),  # the paper's annihilation mask (Alg. 2 l.12-13), dyadic d
+    (0x100, 2048, 192, 0.3, 0.2, 512, 64, 8, 1),     # same, generic d (lazy DIFF tail), Bernoulli start
+    (0x101, 4096, 128, 0.5, 0.05, 2048, 64, 4, 0),   # same on TCPD
 ]
 
 

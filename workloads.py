@@ -20,6 +20,7 @@ import math
 import numpy as np
 
 PCPD = 0  # AA0/0AA->AAA, AA->00, A0<->0A   (eq. (1))
+PMASK_PAPER = 0x100  # variant flag: the paper's own partially correlated annihilation mask
 TCPD = 1  # AAA0/0AAA->AAAA, AAA->000, A0<->0A (BASELINE.json config 5)
 
 INIT_FULL = 0       # all sites occupied
