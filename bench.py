@@ -67,14 +67,22 @@ WIDE_FIXED = 3.0
 
 
 def algorithmic_instr_per_attempt_word(cfg: wl.Config) -> dict:
-    alu_fixed = 40.0 if cfg.variant == wl.PCPD else 46.0
+    alu_fixed = 40.0 if (cfg.variant & 0xff) == wl.PCPD else 46.0
     npd, npp = nplanes_of(cfg.d), nplanes_of(cfg.p)
-    lazy_blocks = 1.0 + blocks_needed_generic(npd) + blocks_needed_generic(npp)   # + the MISC block
-    eager_blocks = 1.0 + (npd + 1) // 2 + (npp + 1) // 2
+    if cfg.variant & wl.PMASK_PAPER:   # the paper's annihilation mask: ANNI block 0 only (two planes ANDed + gate)
+        lazy_blocks = 1.0 + blocks_needed_generic(npd) + 1.0
+        eager_blocks = 1.0 + (npd + 1) // 2 + 1.0
+    else:
+        lazy_blocks = 1.0 + blocks_needed_generic(npd) + blocks_needed_generic(npp)   # + the MISC block
+        eager_blocks = 1.0 + (npd + 1) // 2 + (npp + 1) // 2
     per_block = WIDE_PER_BLOCK + ALU_PER_BLOCK
     fixed = WIDE_FIXED + alu_fixed
     return dict(lazy=fixed + per_block * lazy_blocks, eager=fixed + per_block * eager_blocks,
                 lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=fixed, per_block=per_block)
+
+
+def variant_name(v: int) -> str:
+    return ("PCPD" if (v & 0xff) == wl.PCPD else "TCPD") + ("+paper-pmask" if v & wl.PMASK_PAPER else "")
 
 
 def load_peaks() -> dict:
@@ -181,7 +189,7 @@ def reference_arm(args, cfg: wl.Config) -> None:
                 ms_per_step=1e3 * t_total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="u8", data="synthetic", impl="reference",
                 config=dict(workload=cfg.name, L=cfg.L, n_replicas=cfg.n_replicas, d=cfg.d, p=cfg.p,
-                            variant="PCPD" if cfg.variant == wl.PCPD else "TCPD", sample=sample),
+                            variant=variant_name(cfg.variant), sample=sample),
                 cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
@@ -326,7 +334,7 @@ def ours_arm(args, cfg: wl.Config) -> None:
                     ms_per_step=t_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                     dtype="u64", data="synthetic",
                     config=dict(workload=cfg.name, L=cfg.L, n_replicas=cfg.n_replicas, d=cfg.d, p=cfg.p,
-                                variant="PCPD" if cfg.variant == wl.PCPD else "TCPD", seed=cfg.seed,
+                                variant=variant_name(cfg.variant), seed=cfg.seed,
                                 sweeps_per_step=SWEEPS_PER_STEP, step="pcpd_run(10) + pcpd_density",
                                 schedule=h.schedule_info(), lattice_bytes=cfg.lattice_bytes,
                                 l2="lattice (1 GiB at cfg4) is larger than L2; no flush needed" if cfg.lattice_bytes > 200e6

@@ -59,7 +59,13 @@ CONFIGS = (
     Config("cfg4", PCPD, 1 << 22, 2048, 0.8, 0.12, INIT_FULL, 4, 2000, "log20"),
     Config("cfg5", TCPD, 1 << 20, 1024, 0.5, 0.05, INIT_FULL, 5, 10_000, "log20"),
 )
-BY_NAME = {c.name: c for c in CONFIGS}
+# Not a BASELINE.json config: cfg4's size with the paper's own mask generation (next-row f2, DESIGN.md
+# section 10): dyadic d = 3/4 (the paper's AND/OR recipe) and the partially correlated
+# annihilation mask, p < 1/4.  `bench.py --config cfg4p` measures it.
+EXTRA_CONFIGS = (
+    Config("cfg4p", PCPD | PMASK_PAPER, 1 << 22, 2048, 0.75, 0.12, INIT_FULL, 4, 2000, "log20"),
+)
+BY_NAME = {c.name: c for c in CONFIGS + EXTRA_CONFIGS}
 
 
 def record_times(n_sweeps: int, per_decade: int = 20) -> list[int]:
