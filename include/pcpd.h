@@ -11,7 +11,7 @@
  *   L sites, periodic.  R = n_replicas, W = R/64 words per site.  Word (i, w)
  *   holds replicas 64w .. 64w+63 at site i; bit j <-> replica 64w+j.
  *   CANONICAL order of a host lattice buffer: words[i*W + w].  (The device
- *   layout is private: word-blocked [W/Wb][L][Wb].)
+ *   layout is private: column-major [W][L].)
  *   One sweep = one time unit = L attempted updates per replica.
  *   The update schedule, random streams and mask definition are the contract
  *   C1..C9 of DESIGN.md section 3 (SD2(T_s, D, A) shifted domains, Philox-4x32-10
@@ -91,7 +91,7 @@ PCPD_API int pcpd_set_stream(pcpd_t *h, void *cuda_stream);
 PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant);
 
 /* Same with explicit schedule constants (D | T_s | L, A | D, D >= 2*Rr+3 with
- * Rr = 2 PCPD / 3 TCPD; T_s*Wb*8 bytes must fit the 227 KB shared memory) and
+ * Rr = 2 PCPD / 3 TCPD; T_s*8 bytes (one tile column) must fit the 227 KB shared memory) and
  * a global word offset: the handle simulates word columns
  * word_offset .. word_offset + W - 1 of a larger run (multi-GPU sharding by
  * replica words); columns never interact, so the union of

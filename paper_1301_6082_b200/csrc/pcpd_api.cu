@@ -269,7 +269,7 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        g_launches += launch_sweep(h->P, h->variant, h->Wb, h->stream);
+        g_launches += launch_sweep(h->P, h->variant, h->stream);
         h->sweep += 1;
     }
     return check_launch("sweep kernel");

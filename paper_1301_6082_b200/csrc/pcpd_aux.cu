@@ -1,5 +1,6 @@
 // Init (C8), per-replica particle / pair counts (C9; positional popcount) and
-// canonical <-> word-blocked layout permutation.  sm_100a, HBM-bound streaming
+// canonical <-> device layout permutation.  The device layout is column-major [W][L] (Wb = 1; the
+// Wb parameter of these kernels is the general word-blocked form [W/Wb][L][Wb]).  sm_100a, HBM-bound streaming
 // kernels.  See DESIGN.md section 5.
 #include "pcpd_kernels.cuh"
 

@@ -41,7 +41,8 @@ __device__ __forceinline__ uint64_t lazy_mask(uint64_t rel, const Threshold th, 
 }
 
 // ---------------------------------------------------------------------------
-// One sweep of schedule SD2(Ts, D, A) (C5).  Grid (L/Ts tiles, W/WB word
+// GENERIC FALLBACK (schedules with more than 32 domains per tile; WB = 1 in the column-major
+// layout).  One sweep of schedule SD2(Ts, D, A) (C5).  Grid (L/Ts tiles, W/WB word
 // groups); block = n * WB threads, thread (b, w') owns domain b of word column
 // w' for the whole sweep; the tile lives in shared memory from load to store,
 // so the lattice crosses HBM exactly once in each direction per sweep.
@@ -168,43 +169,31 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
 
 size_t sweep_smem_bytes(uint32_t Ts, int Wb) { return (size_t)Ts * Wb * 8; }
 
-template <int VARIANT, int WB>
+template <int VARIANT>
 static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
 {
-    dim3 grid(P.L / P.Ts, P.W / WB);
-    dim3 block(P.n * WB);
-    sweep_kernel<VARIANT, WB><<<grid, block, sweep_smem_bytes(P.Ts, WB), stream>>>(P);
+    dim3 grid(P.L / P.Ts, P.W);
+    dim3 block(P.n);
+    sweep_kernel<VARIANT, 1><<<grid, block, sweep_smem_bytes(P.Ts, 1), stream>>>(P);
     return 1;
 }
 
-int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream)
+// The production path is the warp-per-(tile, column) kernel of sweep_warp.cu; the block kernel
+// above only serves schedules with more than 32 domains per tile.
+int launch_sweep(const SweepParams &P, int variant, cudaStream_t stream)
 {
-    if (Wb == 1 && sweep_warp_supported(P.Ts, P.D)) return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream);
-    if (variant == 0) {
-        if (Wb == 4) return launch_sweep_t<0, 4>(P, stream);
-        if (Wb == 2) return launch_sweep_t<0, 2>(P, stream);
-        return launch_sweep_t<0, 1>(P, stream);
-    }
-    if (Wb == 4) return launch_sweep_t<1, 4>(P, stream);
-    if (Wb == 2) return launch_sweep_t<1, 2>(P, stream);
-    return launch_sweep_t<1, 1>(P, stream);
-}
-
-template <int VARIANT, int WB>
-static cudaError_t cfg_one()
-{
-    return cudaFuncSetAttribute(sweep_kernel<VARIANT, WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (sweep_warp_supported(P.Ts, P.D))
+        return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream);
+    return variant == 0 ? launch_sweep_t<0>(P, stream) : launch_sweep_t<1>(P, stream);
 }
 
 int configure_kernels()
 {
     cudaError_t e;
-    if ((e = cfg_one<0, 4>()) != cudaSuccess) return (int)e;
-    if ((e = cfg_one<0, 2>()) != cudaSuccess) return (int)e;
-    if ((e = cfg_one<0, 1>()) != cudaSuccess) return (int)e;
-    if ((e = cfg_one<1, 4>()) != cudaSuccess) return (int)e;
-    if ((e = cfg_one<1, 2>()) != cudaSuccess) return (int)e;
-    if ((e = cfg_one<1, 1>()) != cudaSuccess) return (int)e;
+    if ((e = cudaFuncSetAttribute(sweep_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+        return (int)e;
+    if ((e = cudaFuncSetAttribute(sweep_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+        return (int)e;
     return configure_warp_kernels();
 }
 

@@ -19,7 +19,7 @@ struct Threshold {
 };
 
 struct SweepParams {
-    uint64_t *lat;  // device, word-blocked [W/Wb][L][Wb]
+    uint64_t *lat;  // device, column-major [W][L]
     uint32_t L, W;  // W = local word columns of this handle
     uint32_t Ts, D, A, S, n;  // n = Ts / D domains per tile, S = D / A sub-steps
     uint32_t word_offset;     // global index of local column 0
@@ -39,7 +39,7 @@ struct SweepParams {
 };
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.
-int launch_sweep(const SweepParams &P, int variant, int Wb, cudaStream_t stream);
+int launch_sweep(const SweepParams &P, int variant, cudaStream_t stream);
 // warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);

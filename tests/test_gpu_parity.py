@@ -223,3 +223,40 @@ def test_philox_block_via_init_stream(pk):
     o.init(wl.INIT_BERNOULLI)
     assert np.array_equal(lat, o.get_words())
     g.close()
+
+
+def test_error_behaviour_of_the_boundary(pk):
+    """include/pcpd.h: every invalid argument is refused with a message, nothing is silently clamped
+    except T_s > L; the sweep counter refuses to pass 2^32 - 1."""
+    bad = [
+        dict(L=4096, n_replicas=100, d=0.5, p=0.1),            # n_replicas not a multiple of 64
+        dict(L=4096, n_replicas=0, d=0.5, p=0.1),
+        dict(L=4100, n_replicas=64, d=0.5, p=0.1),             # L not a multiple of D
+        dict(L=32, n_replicas=64, d=0.5, p=0.1),               # L < D
+        dict(L=4096, n_replicas=64, d=1.5, p=0.1),
+        dict(L=4096, n_replicas=64, d=0.5, p=float("nan")),
+        dict(L=4096, n_replicas=64, d=0.5, p=0.1, variant=7),  # unknown variant
+        dict(L=4096, n_replicas=64, d=0.5, p=0.25, variant=pk.PMASK_PAPER),   # paper mask needs p < 1/4
+        dict(L=5120, n_replicas=64, d=0.5, p=0.1),             # L % T_s != 0 (T_s = 2048 not clamped: L > T_s)
+        dict(L=4096, n_replicas=64, d=0.5, p=0.1, Ts=2048, D=64, A=5),   # A does not divide D
+        dict(L=4096, n_replicas=64, d=0.5, p=0.1, Ts=2048, D=6, A=2),    # D < 2*Rr + 3
+    ]
+    for kw in bad:
+        kw = dict(dict(seed=1, variant=0), **kw)
+        with pytest.raises(pk.PcpdError) as e:
+            pk.Pcpd(**kw)
+        assert len(str(e.value)) > 20, kw
+    g = pk.Pcpd(1024, 64, 0.5, 0.1, 1, 0)          # T_s clamped to L
+    assert g.schedule_info()["Ts"] == 1024
+    g.sweep = 2 ** 32 - 2
+    g.init(pk.INIT_FULL)
+    assert g.sweep == 0                             # init resets the counter
+    g.sweep = 2 ** 32 - 2
+    g.run(1)
+    with pytest.raises(pk.PcpdError):
+        g.run(1)
+    with pytest.raises(pk.PcpdError):
+        g.sweep = 2 ** 32
+    with pytest.raises(pk.PcpdError):
+        g.init(9)
+    g.close()
