@@ -90,6 +90,10 @@ PCPD_API int pcpd_set_stream(pcpd_t *h, void *cuda_stream);
  * W >= 2^32; unknown variant; allocation failure; no sm_100 device. */
 PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant);
 
+/* Test hook: with the environment variable PCPD_FORCE_BLOCK_KERNEL=1 set at create time the handle
+ * runs the generic block-per-tile sweep kernel instead of the warp-per-tile one (same results, bit
+ * for bit; used by the parity tests to cross-check the two kernels at full size). */
+
 /* Same with explicit schedule constants (D | T_s | L, A | D, D >= 2*Rr+3 with
  * Rr = 2 PCPD / 3 TCPD; T_s*8 bytes (one tile column) must fit the 227 KB shared memory) and
  * a global word offset: the handle simulates word columns

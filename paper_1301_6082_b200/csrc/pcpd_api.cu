@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <atomic>
 #include <new>
@@ -77,6 +78,7 @@ struct pcpd_s {
     uint64_t Td, Tp;
     int Wb;
     uint64_t sweep;
+    bool force_block;  // test hook (env PCPD_FORCE_BLOCK_KERNEL=1 at create): run the generic block kernel
     uint64_t *lat;     // device, word-blocked
     uint32_t *counts;  // device, uint32[R]
     cudaStream_t stream;
@@ -189,6 +191,11 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     h->L = L; h->R = n_replicas; h->W = W; h->d = d; h->p = p; h->seed = seed; h->variant = variant;
     h->Ts = Ts; h->D = D; h->A = A; h->word_offset = word_offset; h->Wb = Wb; h->sweep = 0;
     h->Td = threshold_of(d); h->Tp = threshold_of(p);
+    {
+        const char *fb = getenv("PCPD_FORCE_BLOCK_KERNEL");
+        h->force_block = fb && fb[0] == '1' && !pmask_paper && (uint64_t)(Ts / D) <= 1024 &&
+                         sweep_smem_bytes(Ts, Wb) <= 200 * 1024;
+    }
     h->stream = nullptr;
     h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
     h->counts = (uint32_t *)dev_alloc(4 * n_replicas, h->stream);
@@ -269,7 +276,7 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        g_launches += launch_sweep(h->P, h->variant, h->stream);
+        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream);
         h->sweep += 1;
     }
     return check_launch("sweep kernel");

@@ -39,7 +39,7 @@ struct SweepParams {
 };
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.
-int launch_sweep(const SweepParams &P, int variant, cudaStream_t stream);
+int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream);
 // warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);

@@ -260,3 +260,34 @@ def test_error_behaviour_of_the_boundary(pk):
     with pytest.raises(pk.PcpdError):
         g.init(9)
     g.close()
+
+
+def test_two_independent_kernels_agree_at_full_size(pk, monkeypatch):
+    """Beyond the oracle's horizon (SURVEY.md 8(d) 'self-consistency'): the production warp-per-tile
+    kernel and the generic block-per-tile kernel (different thread mapping, barriers, tile layout,
+    Philox code path and compare code) must give the identical lattice on a full-size config.
+    compute-sanitizer is closed on this pool, so this doubles as the memory-safety check: an
+    out-of-bounds or racing shared-memory access in either kernel would show up as a mismatch."""
+    c = wl.BY_NAME["cfg3"]
+    res = []
+    for force in ("0", "1"):
+        monkeypatch.setenv("PCPD_FORCE_BLOCK_KERNEL", force)
+        g = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
+        g.init(c.init)
+        g.run(3)
+        res.append((g.get_lattice(), g.density(), g.pair_density()))
+        g.close()
+    monkeypatch.delenv("PCPD_FORCE_BLOCK_KERNEL")
+    assert np.array_equal(res[0][0], res[1][0])
+    assert np.array_equal(res[0][1], res[1][1]) and np.array_equal(res[0][2], res[1][2])
+    # and a generic-threshold case with lazy tails on both streams, Bernoulli start
+    res = []
+    for force in ("0", "1"):
+        monkeypatch.setenv("PCPD_FORCE_BLOCK_KERNEL", force)
+        g = pk.Pcpd(1 << 18, 512, 0.8, 0.12, 4, 0)
+        g.init(pk.INIT_BERNOULLI)
+        g.run(5)
+        res.append(g.get_lattice())
+        g.close()
+    monkeypatch.delenv("PCPD_FORCE_BLOCK_KERNEL")
+    assert np.array_equal(res[0], res[1])
