@@ -213,20 +213,37 @@ void oracle_rule_tcpd(uint8_t *qm1, uint8_t *q0, uint8_t *q1, uint8_t *q2, uint8
     }
 }
 
+/* QCPD, the quadruplet contact process with diffusion the paper names as a further model the
+ * algorithm extends to (next-row f4 of SURVEY.md 8(f)), by the same analogy with
+ * Alg. 1 as TCPD (reading G15): AAAA0/0AAAA -> AAAAA each at rate (1-p)(1-d)/2, AAAA -> 0000 at
+ * rate p(1-d), A0 <-> 0A at rate d; footprint {x-1 .. x+4}; diffusion still swaps (x, x+1). */
+void oracle_rule_qcpd(uint8_t *qm1, uint8_t *q0, uint8_t *q1, uint8_t *q2, uint8_t *q3, uint8_t *q4,
+                      int Dm, int Pm, int Fm)
+{
+    if (Dm) {
+        uint8_t tmp = *q0; *q0 = *q1; *q1 = tmp;
+    } else if (*q0 == 1 && *q1 == 1 && *q2 == 1 && *q3 == 1) {
+        if (Pm) { *q0 = 0; *q1 = 0; *q2 = 0; *q3 = 0; }
+        else if (Fm) { *qm1 = 1; }
+        else { *q4 = 1; }
+    }
+}
+
 /* Single attempt on a periodic ring of L sites at site i (literal indexing,
  * reading G2: indices mod L).  Exposed for the master-equation pin P4. */
 void oracle_single_attempt(int variant, uint32_t L, uint8_t *q, uint32_t i,
                            int Dm, int Pm, int Fm)
 {
-    uint32_t im1 = (i + L - 1) % L, i1 = (i + 1) % L, i2 = (i + 2) % L, i3 = (i + 3) % L;
-    if (variant == 0) oracle_rule_pcpd(&q[im1], &q[i], &q[i1], &q[i2], Dm, Pm, Fm);
-    else              oracle_rule_tcpd(&q[im1], &q[i], &q[i1], &q[i2], &q[i3], Dm, Pm, Fm);
+    uint32_t im1 = (i + L - 1) % L, i1 = (i + 1) % L, i2 = (i + 2) % L, i3 = (i + 3) % L, i4 = (i + 4) % L;
+    if (variant == 0)      oracle_rule_pcpd(&q[im1], &q[i], &q[i1], &q[i2], Dm, Pm, Fm);
+    else if (variant == 1) oracle_rule_tcpd(&q[im1], &q[i], &q[i1], &q[i2], &q[i3], Dm, Pm, Fm);
+    else                   oracle_rule_qcpd(&q[im1], &q[i], &q[i1], &q[i2], &q[i3], &q[i4], Dm, Pm, Fm);
 }
 
 /* --------------------------------------------------------------- handle --- */
 typedef struct oracle_t {
     uint32_t L, Ts, D, A;
-    int variant;               /* 0 PCPD, 1 TCPD */
+    int variant;               /* 0 PCPD, 1 TCPD, 2 QCPD */
     int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
     uint64_t Td, Tp, T4p;
     uint64_t seed;
@@ -251,9 +268,9 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
      * paper's partially correlated annihilation mask, which needs p < 1/4. */
     int pmask_paper = (variant & 0x100) ? 1 : 0;
     variant &= ~0x100;
-    if (variant != 0 && variant != 1) return NULL;
+    if (variant != 0 && variant != 1 && variant != 2) return NULL;
     if (pmask_paper && !(p < 0.25)) return NULL;
-    uint32_t Rr = variant == 0 ? 2u : 3u;
+    uint32_t Rr = 2u + (uint32_t)variant;      /* right reach: 2 PCPD, 3 TCPD, 4 QCPD */
     if (L == 0 || L >= ((uint64_t)1 << 32) || nwords == 0) return NULL;
     if (Ts > L) Ts = (uint32_t)L;
     if (D == 0 || A == 0 || Ts == 0) return NULL;
@@ -326,7 +343,7 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
 {
     const uint32_t L = o->L, Ts = o->Ts, D = o->D;
     const uint32_t n = Ts / D;
-    const uint32_t Rr = o->variant == 0 ? 2u : 3u;
+    const uint32_t Rr = 2u + (uint32_t)o->variant;
     const uint32_t w = o->words[k];
 
     /* C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
@@ -361,9 +378,9 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
 
     /* domain-local x' -> tile-local y = (sigma + b*D + x') mod Ts
      *                 -> global   i = (Sigma + tau*Ts + y) mod L           */
-    uint32_t site[5];
-    for (int s = 0; s < 5; ++s) {
-        uint64_t xl = (uint64_t)(x - 1 + s);                 /* x-1 .. x+3 */
+    uint32_t site[6];
+    for (int s = 0; s < 6; ++s) {
+        uint64_t xl = (uint64_t)(x - 1 + s);                 /* x-1 .. x+4 */
         uint64_t y = ((uint64_t)sigma + (uint64_t)b * D + xl) % Ts;
         site[s] = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts + y) % L);
     }
@@ -376,8 +393,11 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
         if (o->variant == 0)
             oracle_rule_pcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]],
                              Dm[j], Pm[j], Fm);
-        else
+        else if (o->variant == 1)
             oracle_rule_tcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]], &q[site[4]],
+                             Dm[j], Pm[j], Fm);
+        else
+            oracle_rule_qcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]], &q[site[4]], &q[site[5]],
                              Dm[j], Pm[j], Fm);
     }
 }
@@ -493,7 +513,7 @@ int oracle_literal_run(int variant, uint32_t L, uint32_t R, double d, double p,
 {
     uint64_t Td = oracle_threshold(d), Tp = oracle_threshold(p);
     if (Td == UINT64_MAX || Tp == UINT64_MAX) return -1;
-    if (L < (variant == 0 ? 4u : 5u)) return -1;      /* reading G18 */
+    if (variant < 0 || variant > 2 || L < 4u + (uint32_t)variant) return -1;      /* reading G18 */
     uint32_t t = 0;
     for (uint32_t rec = 0; rec < n_rec; ++rec) {
         for (; t < rec_times[rec]; ++t)

@@ -120,7 +120,7 @@ def test_P0p_streams_and_words_are_distinct():
 SCHEDULES = [dict(Ts=2048, D=64, A=4), dict(Ts=64, D=64, A=64), dict(Ts=32, D=16, A=2)]
 
 
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
 @pytest.mark.parametrize("sch", SCHEDULES)
 def test_P1_empty_lattice_is_absorbing(variant, sch):
     o = oracle.Oracle(128, 128, 0.3, 0.2, 11, variant, **sch)
@@ -129,7 +129,7 @@ def test_P1_empty_lattice_is_absorbing(variant, sch):
     assert not o.get_words().any() and not o.counts().any()
 
 
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
 @pytest.mark.parametrize("sch", SCHEDULES)
 def test_P2_d_equals_one_conserves_particles(variant, sch):
     o = oracle.Oracle(128, 128, 1.0, 0.3, 12, variant, **sch)
@@ -142,7 +142,7 @@ def test_P2_d_equals_one_conserves_particles(variant, sch):
     assert not np.array_equal(o.get_words(), w0)  # it did move
 
 
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
 def test_P3_isolated_particles_never_react(variant):
     # one particle per replica: count stays 1 for any d, p
     L = 128
@@ -197,7 +197,7 @@ def master_matrix(variant, L, d, p):
     outer neighbour at (1-p)(1-d)/2; diagonal by normalisation."""
     n = 1 << L
     P = [[Fraction(0)] * n for _ in range(n)]
-    k = 2 if variant == wl.PCPD else 3
+    k = 2 + variant  # cluster size: 2 PCPD, 3 TCPD, 4 QCPD
     for s in range(n):
         b = _bits(s, L)
         for i in range(L):
@@ -236,7 +236,8 @@ def oracle_matrix(variant, L, d, p):
     return P
 
 
-@pytest.mark.parametrize("variant,L", [(wl.PCPD, 4), (wl.PCPD, 5), (wl.PCPD, 6), (wl.TCPD, 5), (wl.TCPD, 6)])
+@pytest.mark.parametrize("variant,L", [(wl.PCPD, 4), (wl.PCPD, 5), (wl.PCPD, 6), (wl.TCPD, 5), (wl.TCPD, 6),
+                                       (wl.QCPD, 6), (wl.QCPD, 7)])
 def test_P4_master_equation_enumeration(variant, L):
     d, p = Fraction(3, 10), Fraction(7, 40)
     assert master_matrix(variant, L, d, p) == oracle_matrix(variant, L, d, p)  # exact rationals
@@ -256,7 +257,7 @@ def test_P4_fission_side_follows_alg1():
     assert list(oracle.single_attempt(wl.PCPD, [1, 0, 0, 0, 0, 1], 5, 0, 0, 0)) == [1, 1, 0, 0, 0, 1]
 
 
-@pytest.mark.parametrize("variant,L", [(wl.PCPD, 6), (wl.TCPD, 6)])
+@pytest.mark.parametrize("variant,L", [(wl.PCPD, 6), (wl.TCPD, 6), (wl.QCPD, 6)])
 def test_P4_literal_mode_mean_density_vs_master_equation(variant, L):
     """E[count] after n = 1, 2, 3 time units (n*L attempts) from P^(nL) (floats
     from the exact-rational matrix) vs the literal Alg. 1 Monte Carlo mean."""
@@ -278,7 +279,7 @@ def test_P4_literal_mode_mean_density_vs_master_equation(variant, L):
 
 
 # ------------------------------------------------------------------ P7 ----
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
 def test_P7_run_splitting_loop_order_word_subsets(variant):
     kw = dict(L=256, n_replicas=256, d=0.3, p=0.12, seed=21, variant=variant, Ts=128, D=32, A=4)
     a = oracle.Oracle(**kw)

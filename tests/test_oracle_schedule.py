@@ -195,3 +195,11 @@ def test_P5_paper_pmask_sd2_matches_literal():
     print("P5 paper-pmask z =", np.round(z, 2), "rel =", np.round(rel, 4))
     assert np.all(np.abs(z) < 4.0), (z, rel)
     assert np.all(np.abs(rel) < 0.02), rel
+
+
+@pytest.mark.slow
+def test_P5_qcpd_sd2_matches_literal():
+    times = [1, 2, 4, 8, 16, 32]
+    z, rel, _, _ = _sd2_vs_literal(wl.QCPD, 512, 1024, 0.5, 0.03, times, dict(Ts=2048, D=64, A=4))
+    print("P5 qcpd z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)

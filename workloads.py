@@ -23,6 +23,8 @@ PCPD = 0  # AA0/0AA->AAA, AA->00, A0<->0A   (eq. (1))
 PMASK_PAPER = 0x100  # variant flag: the paper's own partially correlated annihilation mask
 TCPD = 1  # AAA0/0AAA->AAAA, AAA->000, A0<->0A (BASELINE.json config 5)
 
+QCPD = 2  # AAAA0/0AAAA->AAAAA, AAAA->0000, A0<->0A (PAPER.md:21 names it; rule by analogy with Alg. 1)
+
 INIT_FULL = 0       # all sites occupied
 INIT_BERNOULLI = 1  # i.i.d. Bernoulli(1/2) per site per replica from the handle's seed
 INIT_EMPTY = 2      # absorbing state, for tests
