@@ -103,11 +103,11 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
 {
     const int pmask_paper = (variant & PCPD_VARIANT_PMASK_PAPER) ? 1 : 0;
     variant &= ~PCPD_VARIANT_PMASK_PAPER;
-    if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD) {
+    if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD && variant != PCPD_VARIANT_QCPD) {
         fail(PCPD_ERR_ARG, "unknown variant %d", variant);
         return nullptr;
     }
-    const uint32_t Rr = variant == 0 ? 2u : 3u;
+    const uint32_t Rr = 2u + (uint32_t)variant;
     if (n_replicas == 0 || n_replicas % 64) {
         fail(PCPD_ERR_ARG, "n_replicas must be a positive multiple of 64");
         return nullptr;

@@ -114,6 +114,9 @@ SMALL = [
     (0x100, 4096, 256, 0.75, 0.12, 2048, 64, 4, 0),  # the paper's annihilation mask (Alg. 2 l.12-13), dyadic d
     (0x100, 2048, 192, 0.3, 0.2, 512, 64, 8, 1),     # same, generic d (lazy DIFF tail), Bernoulli start
     (0x101, 4096, 128, 0.5, 0.05, 2048, 64, 4, 0),   # same on TCPD
+    (2, 4096, 128, 0.5, 0.03, 2048, 64, 4, 0),       # QCPD, 6-site footprint
+    (2, 1408, 128, 0.3, 0.1, 704, 11, 1, 1),         # QCPD, smallest legal domain D = 11 (n = 64: block kernel)
+    (0x102, 2048, 64, 0.25, 0.05, 1024, 32, 2, 1),   # QCPD with the paper's annihilation mask
 ]
 
 
