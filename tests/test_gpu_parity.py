@@ -294,3 +294,24 @@ def test_two_independent_kernels_agree_at_full_size(pk, monkeypatch):
         g.close()
     monkeypatch.delenv("PCPD_FORCE_BLOCK_KERNEL")
     assert np.array_equal(res[0], res[1])
+
+
+def test_P8_phase_behaviour_smoke(pk):
+    """Qualitative only (pin P8; PAPER.md:41 and Fig. 1, p_c(d = 0.75) = 0.191789(2)):
+    well below p_c the density settles on a plateau (active phase), well above it decays towards the
+    single absorbing state.  Not a parity test - the paper's precision needs L = 2^18 and t ~ 10^7."""
+    L, R, d = 1 << 16, 256, 0.75
+    rho = {}
+    for p in (0.10, 0.30):
+        g = pk.Pcpd(L, R, d, p, 12, pk.PCPD)
+        g.init(pk.INIT_FULL)
+        series = []
+        for _ in range(4):
+            g.run(500)
+            series.append(float(g.density().mean()) / L)
+        rho[p] = series
+        g.close()
+    active, absorbing = rho[0.10], rho[0.30]
+    assert active[-1] > 0.2 and abs(active[-1] - active[-2]) < 0.02 * active[-1]      # plateau
+    assert absorbing[-1] < 0.05 and absorbing[-1] < absorbing[0]                          # decay
+    assert active[-1] > 5 * absorbing[-1]
