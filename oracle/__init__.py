@@ -121,6 +121,7 @@ def paper_pmask(seed, slot, sweep, word, T4p) -> np.ndarray:
     return m
 
 
+CONNECTED = 0x200    # variant flag: the paper's connected multispin lattice (64 lanes = one ring of 64 L sites)
 PMASK_PAPER = 0x100  # variant flag: the paper's own annihilation mask (needs p < 1/4)
 
 

@@ -245,6 +245,7 @@ typedef struct oracle_t {
     uint32_t L, Ts, D, A;
     int variant;               /* 0 PCPD, 1 TCPD, 2 QCPD */
     int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
+    int connected;             /* 1: the paper's connected multispin lattice (C10, below) */
     uint64_t Td, Tp, T4p;
     uint64_t seed;
     uint32_t sweep;            /* C7: state = lattice + sweep counter */
@@ -267,7 +268,9 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     /* variant = base | ORACLE_PMASK_PAPER (0x100): base 0 PCPD / 1 TCPD; the flag selects the
      * paper's partially correlated annihilation mask, which needs p < 1/4. */
     int pmask_paper = (variant & 0x100) ? 1 : 0;
-    variant &= ~0x100;
+    /* | ORACLE_CONNECTED (0x200): the paper's connected multispin lattice, C10. */
+    int connected = (variant & 0x200) ? 1 : 0;
+    variant &= ~0x300;
     if (variant != 0 && variant != 1 && variant != 2) return NULL;
     if (pmask_paper && !(p < 0.25)) return NULL;
     uint32_t Rr = 2u + (uint32_t)variant;      /* right reach: 2 PCPD, 3 TCPD, 4 QCPD */
@@ -282,6 +285,7 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     if (!o) return NULL;
     o->L = (uint32_t)L; o->Ts = Ts; o->D = D; o->A = A; o->variant = variant;
     o->pmask_paper = pmask_paper;
+    o->connected = connected;
     o->T4p = pmask_paper ? oracle_threshold(4.0 * p) : 0;   /* floor(4p * 2^32) < 2^32 since p < 1/4 */
     o->Td = Td; o->Tp = Tp; o->seed = seed; o->sweep = 0; o->nwords = nwords;
     o->words = (uint32_t *)malloc(sizeof(uint32_t) * nwords);
@@ -377,28 +381,38 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
     o->blocks_needed_P += (uint64_t)((needP + 1) / 2);
 
     /* domain-local x' -> tile-local y = (sigma + b*D + x') mod Ts
-     *                 -> global   i = (Sigma + tau*Ts + y) mod L           */
-    uint32_t site[6];
+     *                 -> global   i = (Sigma + tau*Ts + y) mod L
+     * C10 - the paper's CONNECTED multispin lattice ("we connected the N_r
+     * lattices of the classical approach, to form one larger lattice", sites of one register
+     * the maximum distance apart; "the necessary bit-rotations to connect the
+     * multi-spin lattices"; next-row f3 of SURVEY.md 8(f)): the 64 bit-lanes of a word column
+     * are 64 consecutive segments of ONE ring of 64 L sites; the successor of (site L-1, lane j)
+     * is (site 0, lane (j+1) mod 64).  A footprint site whose unreduced index Sigma + tau*Ts + y
+     * passed L therefore belongs, for the strand that has lane j before the wrap, to lane j+1. */
+    uint32_t site[6], lane_shift[6];
     for (int s = 0; s < 6; ++s) {
         uint64_t xl = (uint64_t)(x - 1 + s);                 /* x-1 .. x+4 */
         uint64_t y = ((uint64_t)sigma + (uint64_t)b * D + xl) % Ts;
-        site[s] = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts + y) % L);
+        uint64_t gidx = (uint64_t)Sigma + (uint64_t)tau * Ts + y;   /* < 2L */
+        site[s] = (uint32_t)(gidx % L);
+        lane_shift[s] = (o->connected && gidx >= L) ? 1u : 0u;
     }
 
     for (int j = 0; j < 64; ++j) {
-        uint8_t *q = o->q + ((size_t)k * 64 + j) * L;
+        uint8_t *qs[6];      /* the strand's six footprint sites */
+        for (int s = 0; s < 6; ++s)
+            qs[s] = o->q + ((size_t)k * 64 + ((uint32_t)j + lane_shift[s]) % 64) * L + site[s];
+        /* mask lane j belongs to the strand that is in bit-lane j BEFORE the wrap (the word as
+         * it sits in the register after the bit rotation) */
         /* Fm = mask(1/2) from plane `lo` (C4): U_j < 2^31 <=> top bit of U_j,
          * i.e. lane j of plane 0, is 0.  Fm = 1 => fission LOW (G8). */
         int Fm = ((misc_lo >> j) & 1u) == 0 ? 1 : 0;
         if (o->variant == 0)
-            oracle_rule_pcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]],
-                             Dm[j], Pm[j], Fm);
+            oracle_rule_pcpd(qs[0], qs[1], qs[2], qs[3], Dm[j], Pm[j], Fm);
         else if (o->variant == 1)
-            oracle_rule_tcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]], &q[site[4]],
-                             Dm[j], Pm[j], Fm);
+            oracle_rule_tcpd(qs[0], qs[1], qs[2], qs[3], qs[4], Dm[j], Pm[j], Fm);
         else
-            oracle_rule_qcpd(&q[site[0]], &q[site[1]], &q[site[2]], &q[site[3]], &q[site[4]], &q[site[5]],
-                             Dm[j], Pm[j], Fm);
+            oracle_rule_qcpd(qs[0], qs[1], qs[2], qs[3], qs[4], qs[5], Dm[j], Pm[j], Fm);
     }
 }
 

@@ -379,3 +379,53 @@ def test_P9_paper_pmask_mode_in_run():
     # same positions and fission bits, different annihilation masks -> different states
     assert not np.array_equal(a.get_words(), b.get_words())
     assert a.counts().min() < 64  # something was annihilated at p = 0.2
+
+
+# ----------------------------------------------------------------- P10 ----
+# The paper's connected multispin lattice (next-row f3): the 64 bit-lanes of a
+# word column are 64 consecutive segments of ONE ring of 64 L sites, joined by a bit rotation at the
+# seam.  Pinned to what that sentence fixes: a particle is a random walker on the long ring (its
+# strand position lane*L + site moves by small steps only, also across the seam, and it does cross);
+# d = 1 conserves the particle number of the RING (the sum over the 64 lanes), not of a lane.
+def test_P10_connected_lattice_single_walker_crosses_the_seam():
+    L = 256
+    o = oracle.Oracle(L, 64, 1.0, 0.3, 17, oracle.CONNECTED, Ts=256, D=64, A=4)
+    w = np.zeros((L, 1), np.uint64)
+    w[L - 1, 0] = np.uint64(1) << np.uint64(5)
+    o.set_words(w)
+    ring = 64 * L
+    pos, lanes = 5 * L + (L - 1), {5}
+    for _ in range(300):
+        o.run(1)
+        g = o.get_words()[:, 0]
+        sites = np.nonzero(g)[0]
+        assert len(sites) == 1 and bin(int(g[sites[0]])).count("1") == 1      # still exactly one particle
+        lane = int(g[sites[0]]).bit_length() - 1
+        new = lane * L + int(sites[0])
+        step = (new - pos + ring // 2) % ring - ring // 2
+        assert abs(step) < L // 4, (pos, new)      # a wrongly wired seam makes the walker jump by ~L or 2L
+        pos = new
+        lanes.add(lane)
+    assert len(lanes) >= 2                        # it did cross the seam
+
+
+def test_P10_connected_lattice_conserves_ring_not_lane():
+    L = 128
+    kw = dict(L=L, n_replicas=128, d=1.0, p=0.2, seed=23, Ts=128, D=32, A=4)
+    w0 = wl.random_lattice_words(L, 2, 0.3, seed=5)
+    a = oracle.Oracle(variant=oracle.CONNECTED, **kw)
+    b = oracle.Oracle(variant=0, **kw)
+    for o in (a, b):
+        o.set_words(w0)
+    c0 = a.counts().astype(np.int64)
+    a.run(20)
+    b.run(20)
+    ca, cb = a.counts().astype(np.int64), b.counts().astype(np.int64)
+    assert np.array_equal(cb, c0)                                   # independent lanes: each lane conserved
+    assert np.array_equal(ca.reshape(2, 64).sum(axis=1), c0.reshape(2, 64).sum(axis=1))   # ring conserved
+    assert not np.array_equal(ca, c0)                               # ... but particles changed lanes
+    # empty lattice is absorbing in this mode too
+    e = oracle.Oracle(variant=oracle.CONNECTED, **dict(kw, d=0.3))
+    e.init(wl.INIT_EMPTY)
+    e.run(3)
+    assert not e.get_words().any()

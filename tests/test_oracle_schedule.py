@@ -203,3 +203,29 @@ def test_P5_qcpd_sd2_matches_literal():
     z, rel, _, _ = _sd2_vs_literal(wl.QCPD, 512, 1024, 0.5, 0.03, times, dict(Ts=2048, D=64, A=4))
     print("P5 qcpd z =", np.round(z, 2), "rel =", np.round(rel, 4))
     assert np.all(np.abs(z) < 4.0), (z, rel)
+
+
+@pytest.mark.slow
+def test_P5_connected_lattice_matches_literal_on_the_long_ring():
+    """Connected multispin lattice: one word column = one ring of 64 L sites.  Its
+    density decay must agree with the literal Algorithm 1 run on a ring of that length (the paper:
+    "we found no bias" when the sites of a register are L apart).  Words / rings are the samples."""
+    L, W = 256, 32
+    times = [1, 2, 4, 8, 16, 32, 64]
+    o = oracle.Oracle(L, 64 * W, 0.5, 0.15, 9, wl.PCPD | oracle.CONNECTED, Ts=256, D=64, A=4)
+    o.init(wl.INIT_FULL)
+    sd2, prev = [], 0
+    for t in times:
+        o.run(t - prev)
+        prev = t
+        sd2.append(o.counts().astype(np.float64).reshape(W, 64).sum(axis=1) / (64 * L))
+    sd2 = np.array(sd2)
+    lit, _ = oracle.literal_run(wl.PCPD, 64 * L, W, 0.5, 0.15, 1009, np.ones((W, 64 * L), np.uint8), times)
+    lit = lit.astype(np.float64) / (64 * L)
+    m_s, e_s = sd2.mean(axis=1), sd2.std(axis=1, ddof=1) / W ** 0.5
+    m_l, e_l = lit.mean(axis=1), lit.std(axis=1, ddof=1) / W ** 0.5
+    z = (m_s - m_l) / np.sqrt(e_s ** 2 + e_l ** 2)
+    rel = m_s / m_l - 1
+    print("P5 connected z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)
+    assert np.all(np.abs(rel) < 0.02), rel
