@@ -65,6 +65,13 @@ enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1, PCPD_VARIANT_Q
  * Costs 3 Philox blocks per attempt-word when d is a short dyadic (d = 1/2, 1/4, 3/4: the
  * paper's AND/OR recipe for d, is what C3 reduces to for such d). */
 #define PCPD_VARIANT_PMASK_PAPER 0x100
+/* Flag to OR into `variant`: the PAPER's CONNECTED multispin lattice instead of
+ * 64 independent replicas per word: the 64 bit-lanes of a word column are 64 consecutive segments of
+ * ONE periodic lattice of 64*L sites (strand position lane*L + site); the successor of (site L-1,
+ * lane j) is (site 0, lane (j+1) mod 64).  n_replicas/64 such lattices are simulated; pcpd_density
+ * still returns per-lane counts (sum 64 consecutive entries for a lattice's particle number).
+ * Schedule, streams and masks are unchanged: an attempt-word updates 64 positions L sites apart. */
+#define PCPD_VARIANT_CONNECTED 0x200
 enum pcpd_init_mode { PCPD_INIT_FULL = 0, PCPD_INIT_BERNOULLI = 1, PCPD_INIT_EMPTY = 2 };
 
 /* Default schedule constants of SD2 (C5). */

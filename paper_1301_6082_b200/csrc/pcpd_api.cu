@@ -102,7 +102,8 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
                        uint32_t D, uint32_t A, uint64_t word_offset)
 {
     const int pmask_paper = (variant & PCPD_VARIANT_PMASK_PAPER) ? 1 : 0;
-    variant &= ~PCPD_VARIANT_PMASK_PAPER;
+    const int connected = (variant & PCPD_VARIANT_CONNECTED) ? 1 : 0;
+    variant &= ~(PCPD_VARIANT_PMASK_PAPER | PCPD_VARIANT_CONNECTED);
     if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD && variant != PCPD_VARIANT_QCPD) {
         fail(PCPD_ERR_ARG, "unknown variant %d", variant);
         return nullptr;
@@ -213,6 +214,7 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     P.thd = make_threshold(h->Td);
     P.thp = make_threshold(h->Tp);
     P.rk = make_round_keys(seed);
+    P.connected = (uint32_t)connected;
     P.pmask_paper = (uint32_t)pmask_paper;
     P.T4p = pmask_paper ? (uint32_t)threshold_of(4.0 * p) : 0u;   // < 2^32 because p < 1/4
     for (int k = 0; k < 32; ++k) {

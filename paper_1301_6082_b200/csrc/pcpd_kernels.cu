@@ -80,9 +80,10 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
         }
     } else {
         for (uint32_t y = tid; y < Ts; y += nthr) {
-            uint32_t i = start + y;
-            if (i >= L) i -= L;
-            tile[y] = g[i];
+            uint32_t i = start + y, rot = 0;
+            if (i >= L) { i -= L; rot = P.connected; }  // connected multispin lattice (C10): bit rotation past the wrap
+            const uint64_t v = g[i];
+            tile[y] = (v >> rot) | (v << ((64u - rot) & 63u));
         }
     }
     __syncthreads();
@@ -168,9 +169,10 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
         }
     } else {
         for (uint32_t y = tid; y < Ts; y += nthr) {
-            uint32_t i = start + y;
-            if (i >= L) i -= L;
-            g[i] = tile[y];
+            uint32_t i = start + y, rot = 0;
+            if (i >= L) { i -= L; rot = P.connected; }
+            const uint64_t v = tile[y];
+            g[i] = (v << rot) | (v >> ((64u - rot) & 63u));
         }
     }
 }

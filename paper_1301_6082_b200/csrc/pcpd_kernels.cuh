@@ -35,6 +35,7 @@ struct SweepParams {
     // (tb_(-1) = tb_32 = 0); stopping after M blocks closes the sum with cl[M] = -tb_(2M-1).
     int32_t sd[34], sp[34];
     int32_t cld[18], clp[18];
+    uint32_t connected;       // 1: connected multispin lattice: words of tile sites past the ring wrap are bit-rotated (C10)
     uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
 };
 

@@ -136,6 +136,13 @@ __device__ __forceinline__ void philox_blocks(const uint32_t (&c3in)[N], const P
     for (int i = 0; i < N; ++i) out[i] = U4{c0[i], c1[i], c2[i], c3[i]};
 }
 
+// Connected multispin lattice (C10): the successor of (site L-1, lane j) is
+// (site 0, lane j+1), so the words of the tile sites that lie past the ring wrap are rotated right by
+// one bit when the tile is loaded (bit j of the tile word = the strand that is in lane j before the
+// wrap) and rotated back when it is stored.  r is 0 or 1.
+__device__ __forceinline__ uint64_t rotr64(uint64_t v, uint32_t r) { return (v >> r) | (v << ((64u - r) & 63u)); }
+__device__ __forceinline__ uint64_t rotl64(uint64_t v, uint32_t r) { return (v << r) | (v >> ((64u - r) & 63u)); }
+
 // 64-lane mask state as two 32-bit halves.
 struct Mask2 {
     uint32_t lo, hi;
@@ -200,6 +207,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
     uint64_t *buf = smem + (size_t)warp * stride;
     const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
+    const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
     const uint32_t odd = vec ? (start & 1u) : 0u;
     uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
     if (vec) {
@@ -212,11 +220,21 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             if (i >= L) i -= L;
             b2[pi] = g2[i >> 1];
         }
+        if (conn && s0 + 2 * npairs > L) {
+            // connected lattice: rotate the words past the ring wrap in place (L and s0 are even, so
+            // both words of a pair lie on the same side of the wrap)
+            __syncwarp();
+            for (uint32_t k2 = (L - s0) + lane; k2 < 2 * npairs; k2 += 32) buf[k2] = rotr64(buf[k2], 1u);
+        }
     } else {
         for (uint32_t y = lane; y < Ts; y += 32) {
             uint32_t i = start + y;
             if (i >= L) i -= L;
             tile[y] = g[i];
+        }
+        if (conn && start + Ts > L) {
+            __syncwarp();
+            for (uint32_t y = (L - start) + lane; y < Ts; y += 32) tile[y] = rotr64(tile[y], 1u);
         }
     }
     __syncwarp();
@@ -358,6 +376,14 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     }
 
     // ---- store the tile ----
+    if (conn) {  // connected lattice: rotate the words past the ring wrap back (see the load)
+        const uint32_t first = vec ? (start - odd) : start, nw = vec ? 2 * (Ts / 2 + odd) : Ts;
+        uint64_t *base = vec ? buf : tile;
+        if (first + nw > L) {
+            for (uint32_t k2 = (L - first) + lane; k2 < nw; k2 += 32) base[k2] = rotl64(base[k2], 1u);
+            __syncwarp();
+        }
+    }
     if (vec) {
         const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
         ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
