@@ -59,7 +59,7 @@ def nplanes_of(q: float) -> int:
 
 # Per-block and fixed thread-instruction counts of the sweep kernel's own SASS (sweep_warp.cu, nvcc 12.9):
 # one strength-reduced Philox-4x32-10 block = 16 IMAD.WIDE.U32 + 18 LOP3; MSB-first compare of its two planes
-# = 8 LOP3 (2 per plane per 32-lane half in the minimal masked form; the kernel's branch-free form uses 10);
+# = 8 instructions (per plane and 32-lane half one LOP3 for the und chain + one 32-bit IMAD for the signed-sum lt);
 # per attempt: 2 IMAD.WIDE (slot constants) + 1 IMAD.HI (position) and ~40 logic/address ops (rule 22,
 # position/seam/address 12, tail masks 6; TCPD +6).
 WIDE_PER_BLOCK, ALU_PER_BLOCK = 16.0, 18.0 + 8.0
