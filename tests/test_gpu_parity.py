@@ -319,3 +319,23 @@ def test_P8_phase_behaviour_smoke(pk):
     assert active[-1] > 0.2 and abs(active[-1] - active[-2]) < 0.02 * active[-1]      # plateau
     assert absorbing[-1] < 0.05 and absorbing[-1] < absorbing[0]                          # decay
     assert active[-1] > 5 * absorbing[-1]
+
+
+LONG = os.environ.get("PCPD_LONG_PARITY") == "1"
+
+
+@pytest.mark.skipif(not LONG, reason="long parity run (oracle needs ~40 min of host time): set PCPD_LONG_PARITY=1")
+@pytest.mark.parametrize("name,words,times", [
+    ("cfg2", None, "all"),                                  # the whole run: all 4 columns, every record time up to 10^4
+    ("cfg3", [0, 16, 31], [1, 2, 4, 8, 16, 32, 64]),
+    ("cfg5", [0, 8, 15], [1, 2, 4, 8, 16, 32, 64]),
+    ("cfg4", [0, 31], [1, 2, 4, 8, 16, 32]),
+])
+def test_long_parity_protocol(pk, name, words, times):
+    """SURVEY.md 8(d) parity protocol beyond the default suite's horizon: cfg2 in full (lattice and counts at every
+    log-spaced record time of the 10^4 sweeps), cfg3/4/5 on sampled word columns out to t = 64 (32)."""
+    c = wl.BY_NAME[name]
+    kw = dict(L=c.L, n_replicas=c.n_replicas, d=c.d, p=c.p, seed=c.seed, variant=c.variant)
+    if times == "all":
+        times = [t for t in wl.record_times(c.sweeps) if t > 0]
+    gpu_check(pk, kw, {}, c.init, times, words=words)
