@@ -154,10 +154,15 @@ PCPD_API uint64_t pcpd_launch_count(void);
 
 /* ---- roofline microbenchmarks -----------------------
  * Runs `iters` dependent-chain iterations of one instruction mix on every SM
- * and returns the achieved rate in out_rate (thread-instructions per second,
- * or Philox blocks per second for kind 3), timed with CUDA events.
- * kind 0: LOP3 only; 1: IMAD.WIDE.U32 + LOP3 pairs (a Philox round's mix; rate
- * counts both); 2: 32-bit IMAD only; 3: Philox-4x32-10 blocks. */
+ * (2048 threads per SM, 8 independent chains per thread) and returns the achieved
+ * rate in out_rate (thread-instructions per second, or Philox blocks per second
+ * for kinds 3 and 7), timed with CUDA events, best of 3.
+ * kind 0: LOP3 only; 1: IMAD.WIDE.U32 + LOP3 1:1 (a Philox round's mix; rate counts
+ * both); 2: 32-bit IMAD only; 3: Philox-4x32-10 blocks; 4: LOP3 + 32-bit IMAD 1:1 on
+ * independent chains (do the ALU and FMA pipes co-issue?); 5: IMAD.WIDE.U32 + 3 LOP3
+ * (the sweep kernel's mix: bench.py's roofline peak); 6: IMAD.HI.U32 only;
+ * 7: Philox with mul.hi + mad.lo written separately (ptxas fuses them back).
+ * PCPD_ERR_ARG for another kind, iters == 0 or a NULL out pointer. */
 PCPD_API int pcpd_microbench(int kind, uint32_t iters, double *out_rate);
 
 #ifdef __cplusplus

@@ -422,7 +422,6 @@ int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks)
 {
     if (ntasks < 148ull * 14) return 1;    // small problem: one warp per block so that the warps spread over all SMs
     const size_t per = warp_smem_bytes(Ts, 1);
-    if (14 * per <= 113 * 1024) return 14; // 2 blocks x 14 warps per SM at T_s = 1024 (2 x (114912 + 1024) B)
     if (7 * per <= 113 * 1024) return 7;   // 2 blocks x 7 warps per SM at T_s = 2048 (2 x (114800 + 1024) B)
     return 1;
 }
@@ -470,16 +469,10 @@ static int warp_op_d(int nud, int nup, const SweepParams *P, cudaStream_t stream
 static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams *P, cudaStream_t stream)
 {
     if (variant == 2)
-        return wpb == 14  ? warp_op_d<2, 14>(nud, nup, P, stream)
-               : wpb == 7 ? warp_op_d<2, 7>(nud, nup, P, stream)
-                          : warp_op_d<2, 1>(nud, nup, P, stream);
+        return wpb == 7 ? warp_op_d<2, 7>(nud, nup, P, stream) : warp_op_d<2, 1>(nud, nup, P, stream);
     if (variant == 0)
-        return wpb == 14  ? warp_op_d<0, 14>(nud, nup, P, stream)
-               : wpb == 7 ? warp_op_d<0, 7>(nud, nup, P, stream)
-                          : warp_op_d<0, 1>(nud, nup, P, stream);
-    return wpb == 14  ? warp_op_d<1, 14>(nud, nup, P, stream)
-           : wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream)
-                      : warp_op_d<1, 1>(nud, nup, P, stream);
+        return wpb == 7 ? warp_op_d<0, 7>(nud, nup, P, stream) : warp_op_d<0, 1>(nud, nup, P, stream);
+    return wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream) : warp_op_d<1, 1>(nud, nup, P, stream);
 }
 
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
@@ -490,7 +483,7 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
 
 int configure_warp_kernels()
 {
-    const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[4] = {-1, 0, 1, PCPD_NUP_BIG}, wpbs[3] = {14, 7, 1};
+    const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[4] = {-1, 0, 1, PCPD_NUP_BIG}, wpbs[2] = {7, 1};
     for (int variant = 0; variant < 3; ++variant)
         for (int wpb : wpbs)
             for (int nud : nuds)
