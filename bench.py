@@ -161,9 +161,18 @@ def oracle_sample_rate(cfg: wl.Config, L_sample: int, n_cols: int, sweeps: int =
     with ThreadPoolExecutor(n_cols) as ex:
         list(ex.map(lambda o: o.run(sweeps), handles))
     dt = time.perf_counter() - t0
+    # the oracle's instrumentation: Philox blocks per attempt-word a lazy evaluation needs to decide all 64
+    # lanes of both masks (+ the MISC block); deterministic for a seed, does not influence any result
+    global LAST_ORACLE_LAZY_BLOCKS
+    st = [o.stats() for o in handles]
+    aw = sum(x["attempt_words"] for x in st)
+    LAST_ORACLE_LAZY_BLOCKS = (1.0 + sum(x["blocks_needed_D"] + x["blocks_needed_P"] for x in st) / aw) if aw else None
     for o in handles:
         o.close()
     return L_sample * 64.0 * n_cols * sweeps / dt, dt
+
+
+LAST_ORACLE_LAZY_BLOCKS = None
 
 
 def reference_arm(args, cfg: wl.Config) -> None:
@@ -341,7 +350,8 @@ def ours_arm(args, cfg: wl.Config) -> None:
                                 else "lattice smaller than L2 (correctness config)",
                                 init_ms=init_ms, density_ms=density_ms, parallelism=f"replica-word shards x{world}"),
                     roofline=roof,
-                    cpu_baseline=dict(value=cpu_rate, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                    cpu_baseline=dict(value=cpu_rate, unit=UNIT, cores=cores, kind="oracle", sample=sample,
+                                      lazy_blocks_per_attempt_word=LAST_ORACLE_LAZY_BLOCKS),
                     e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=cfg.lattice_bytes,
                              d2h_bytes_per_step=4 * cfg.n_replicas, steps=e2e_steps, wall_s=wall),
                     gpu_launches=int(launches), clocks=clocks)
