@@ -8,6 +8,8 @@ P5: SD2 vs the literal Algorithm 1, mean density at log-spaced
 times - the paper's own way of validating a modified site selection
 (PAPER.md:191-197).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -229,3 +231,47 @@ def test_P5_connected_lattice_matches_literal_on_the_long_ring():
     print("P5 connected z =", np.round(z, 2), "rel =", np.round(rel, 4))
     assert np.all(np.abs(z) < 4.0), (z, rel)
     assert np.all(np.abs(rel) < 0.02), rel
+
+
+@pytest.mark.skipif(os.environ.get("PCPD_LONG_PARITY") != "1", reason="high-statistics bias run (minutes of CPU): set PCPD_LONG_PARITY=1")
+def test_P5_high_statistics_bias_of_the_default_schedule():
+    """The paper's own validation of a parallel schedule at higher statistics: SD2(2048, 64, 4)
+    in its production shape (32 domains per tile) against the literal Algorithm 1, 8192 replicas each, t <= 256.
+    Prints the relative deviation and its error; asserts |z| < 4 and |rel| < 0.5 %."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    L, R, d, p = 4096, 8192, 0.5, 0.15
+    W = R // 64
+    times = [1, 2, 4, 8, 16, 32, 64, 128, 256]
+    nthr = max(1, min(os.cpu_count() or 1, 16))
+
+    def sd2(words):
+        o = oracle.Oracle(L, R, d, p, 7, wl.PCPD, Ts=2048, D=64, A=4, words=list(words))
+        o.init(wl.INIT_FULL)
+        out, prev = [], 0
+        for t in times:
+            o.run(t - prev)
+            prev = t
+            out.append(o.counts().astype(np.float64).reshape(len(words), 64).mean(axis=1) / L)
+        return np.array(out)                                   # [n_t, len(words)]
+
+    def lit(chunk):
+        r0, r1 = chunk
+        c, _ = oracle.literal_run(wl.PCPD, L, r1 - r0, d, p, 1007 + r0, np.ones((r1 - r0, L), np.uint8), times)
+        return c.astype(np.float64) / L                        # [n_t, r1-r0]
+
+    wchunks = np.array_split(np.arange(W), nthr)
+    rchunks = [(int(a[0]) * 64, (int(a[-1]) + 1) * 64) for a in wchunks]
+    with ThreadPoolExecutor(nthr) as ex:
+        s = np.concatenate(list(ex.map(sd2, wchunks)), axis=1)     # [n_t, W]   words are the samples (G12)
+        l = np.concatenate(list(ex.map(lit, rchunks)), axis=1)     # [n_t, R]
+    m_s, e_s = s.mean(axis=1), s.std(axis=1, ddof=1) / W ** 0.5
+    m_l, e_l = l.mean(axis=1), l.std(axis=1, ddof=1) / R ** 0.5
+    z = (m_s - m_l) / np.sqrt(e_s ** 2 + e_l ** 2)
+    rel = m_s / m_l - 1
+    err = np.sqrt(e_s ** 2 + e_l ** 2) / m_l
+    print("P5 high statistics: t =", times)
+    print("  rel =", np.round(rel, 5))
+    print("  +/- =", np.round(err, 5))
+    print("  z   =", np.round(z, 2))
+    assert np.all(np.abs(z) < 4.0) and np.all(np.abs(rel) < 0.005), (z, rel)
