@@ -20,7 +20,7 @@ thread_local char g_err[512] = "";
 std::atomic<uint64_t> g_launches{0};
 pcpd_alloc_fn g_alloc = nullptr;
 pcpd_free_fn g_free = nullptr;
-bool g_configured = false;
+bool g_configured[64] = {};  // per device: the opt-in shared-memory attribute is per context
 
 int fail(int code, const char *fmt, ...)
 {
@@ -175,13 +175,17 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_DEVICE, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor);
         return nullptr;
     }
-    if (!g_configured) {
+    if (dev < 0 || dev >= 64) {
+        fail(PCPD_ERR_DEVICE, "device index %d out of range", dev);
+        return nullptr;
+    }
+    if (!g_configured[dev]) {
         const int rc = configure_kernels();
         if (rc != 0) {
             cuda_fail((cudaError_t)rc, "cudaFuncSetAttribute");
             return nullptr;
         }
-        g_configured = true;
+        g_configured[dev] = true;
     }
 
     pcpd_s *h = new (std::nothrow) pcpd_s();
