@@ -63,6 +63,8 @@ def lib() -> C.CDLL:
         L.oracle_set_sweep.restype = None
         L.oracle_thresholds.argtypes = [C.c_void_p, u64p, u64p]
         L.oracle_thresholds.restype = None
+        L.oracle_set_word_probabilities.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.c_double]
+        L.oracle_set_word_probabilities.restype = C.c_int
         L.oracle_stats.argtypes = [C.c_void_p, u64p]
         L.oracle_stats.restype = None
         L.oracle_init.argtypes = [C.c_void_p, C.c_int]
@@ -176,6 +178,11 @@ class Oracle:
         a, b = C.c_uint64(), C.c_uint64()
         lib().oracle_thresholds(self._h, C.byref(a), C.byref(b))
         return a.value, b.value
+
+    def set_word_probabilities(self, k, d, p):
+        """Column k (index into `words`) uses (d, p) from now on (oracle_set_word_probabilities, C11)."""
+        if lib().oracle_set_word_probabilities(self._h, k, float(d), float(p)) != 0:
+            raise ValueError("oracle_set_word_probabilities: invalid arguments")
 
     def stats(self) -> dict:
         s = np.zeros(5, dtype=np.uint64)

@@ -26,6 +26,8 @@
  *                                 lane probability p, word-wide gate 4p, lanes
  *                                 independent 1/4-bits given the gate, pair
  *                                 probability p/4; P5 bias check vs literal Alg. 1
+ *   oracle_set_word_probabilities  P11 column k of a per-word run == column k of the uniform
+ *                                 run with (d_k, p_k), bit for bit
  *   oracle_run (schedule SD2) P5  vs literal Alg. 1 (statistical), P6 exact toy
  *                                 operator, P7 run splitting / loop order /
  *                                 word subsets
@@ -247,6 +249,7 @@ typedef struct oracle_t {
     int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
     int connected;             /* 1: the paper's connected multispin lattice (C10, below) */
     uint64_t Td, Tp, T4p;
+    uint64_t *Td_w, *Tp_w;     /* per simulated word column (index k): thresholds in force (C11) */
     uint64_t seed;
     uint32_t sweep;            /* C7: state = lattice + sweep counter */
     uint32_t nwords;           /* word columns simulated (subset of the full run) */
@@ -289,8 +292,14 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     o->T4p = pmask_paper ? oracle_threshold(4.0 * p) : 0;   /* floor(4p * 2^32) < 2^32 since p < 1/4 */
     o->Td = Td; o->Tp = Tp; o->seed = seed; o->sweep = 0; o->nwords = nwords;
     o->words = (uint32_t *)malloc(sizeof(uint32_t) * nwords);
+    o->Td_w = (uint64_t *)malloc(sizeof(uint64_t) * nwords);
+    o->Tp_w = (uint64_t *)malloc(sizeof(uint64_t) * nwords);
+    if (o->Td_w && o->Tp_w)
+        for (uint32_t k = 0; k < nwords; ++k) { o->Td_w[k] = Td; o->Tp_w[k] = Tp; }
     o->q = (uint8_t *)calloc((size_t)nwords * 64 * (size_t)L, 1);
-    if (!o->words || !o->q) { free(o->words); free(o->q); free(o); return NULL; }
+    if (!o->words || !o->q || !o->Td_w || !o->Tp_w) {
+        free(o->words); free(o->q); free(o->Td_w); free(o->Tp_w); free(o); return NULL;
+    }
     memcpy(o->words, words, sizeof(uint32_t) * nwords);
     return o;
 }
@@ -298,13 +307,28 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
 void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
-    free(o->words); free(o->q); free(o);
+    free(o->words); free(o->q); free(o->Td_w); free(o->Tp_w); free(o);
 }
 
 void oracle_set_reverse_order(oracle_t *o, int rev) { o->reverse_order = rev; }
 uint32_t oracle_sweep(const oracle_t *o) { return o->sweep; }
 void oracle_set_sweep(oracle_t *o, uint32_t t) { o->sweep = t; }
 void oracle_thresholds(const oracle_t *o, uint64_t *Td, uint64_t *Tp) { *Td = o->Td; *Tp = o->Tp; }
+
+/* C11 - per-word-column probabilities (next-row f4 of SURVEY.md 8(f): one run scans p across p_c,
+ * the paper's production use is many runs per p value): simulated column k uses
+ * d_k, p_k, i.e. thresholds floor(d_k 2^32), floor(p_k 2^32); everything else (schedule, streams,
+ * keyed by the global word index) is unchanged, so column k evolves exactly as it would in a
+ * uniform run with (d_k, p_k).  Not available with the paper's annihilation mask.  Returns -1 on
+ * invalid arguments. */
+int oracle_set_word_probabilities(oracle_t *o, uint32_t k, double d, double p)
+{
+    if (!o || k >= o->nwords || o->pmask_paper) return -1;
+    uint64_t Td = oracle_threshold(d), Tp = oracle_threshold(p);
+    if (Td == UINT64_MAX || Tp == UINT64_MAX) return -1;
+    o->Td_w[k] = Td; o->Tp_w[k] = Tp;
+    return 0;
+}
 
 void oracle_stats(const oracle_t *o, uint64_t out[5])
 {
@@ -372,9 +396,9 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
 
     uint8_t Dm[64], Pm[64];
     int needD = 0, needP = 0;
-    bernoulli_lanes(o->seed, g, t, w, STREAM_DIFF, o->Td, Dm, &needD);
+    bernoulli_lanes(o->seed, g, t, w, STREAM_DIFF, o->Td_w[k], Dm, &needD);
     if (o->pmask_paper) { oracle_paper_pmask(o->seed, g, t, w, o->T4p, Pm); needP = 2; }
-    else bernoulli_lanes(o->seed, g, t, w, STREAM_ANNI, o->Tp, Pm, &needP);
+    else bernoulli_lanes(o->seed, g, t, w, STREAM_ANNI, o->Tp_w[k], Pm, &needP);
     o->n_attempt_words += 1;
     o->planes_needed_D += (uint64_t)needD; o->planes_needed_P += (uint64_t)needP;
     o->blocks_needed_D += (uint64_t)((needD + 1) / 2);

@@ -429,3 +429,27 @@ def test_P10_connected_lattice_conserves_ring_not_lane():
     e.init(wl.INIT_EMPTY)
     e.run(3)
     assert not e.get_words().any()
+
+
+# ----------------------------------------------------------------- P11 ----
+def test_P11_per_word_probabilities_equal_uniform_runs():
+    """C11 (next-row f4): with per-word-column probabilities, column k evolves exactly as in a uniform run
+    with (d_k, p_k) - columns never interact and all streams are keyed by the global word index."""
+    L, W = 256, 4
+    ds, ps = [0.5, 0.1, 0.8, 1.0], [0.15, 0.09, 0.0, 0.3]
+    sch = dict(Ts=128, D=32, A=4)
+    o = oracle.Oracle(L, 64 * W, 0.25, 0.25, 77, wl.PCPD, **sch)
+    for k in range(W):
+        o.set_word_probabilities(k, ds[k], ps[k])
+    o.init(wl.INIT_BERNOULLI)
+    o.run(6)
+    got = o.get_words()
+    for k in range(W):
+        u = oracle.Oracle(L, 64 * W, ds[k], ps[k], 77, wl.PCPD, words=[k], **sch)
+        u.init(wl.INIT_BERNOULLI)
+        u.run(6)
+        assert np.array_equal(u.get_words()[:, 0], got[:, k]), k
+    with pytest.raises(ValueError):
+        o.set_word_probabilities(W, 0.5, 0.1)
+    with pytest.raises(ValueError):
+        o.set_word_probabilities(0, 1.5, 0.1)
