@@ -113,6 +113,15 @@ PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p
 PCPD_API pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant,
                        uint32_t T_s, uint32_t D, uint32_t A, uint64_t word_offset);
 
+/* Per-word-column probabilities (one run scans p across p_c; contract C11 of DESIGN.md): word column w of the
+ * handle (global column word_offset + w) uses d_w[w], p_w[w] - HOST arrays of n_replicas/64 doubles, copied at
+ * create time - instead of one (d, p); everything else is as in pcpd_create_ex, and column w evolves bit for bit
+ * as it would in a uniform run with (d_w[w], p_w[w]).  Errors as pcpd_create_ex, plus: NULL arrays, any entry
+ * outside [0,1] or NaN, the PCPD_VARIANT_PMASK_PAPER flag (not available in this mode), more than 32 domains per
+ * tile (T_s / D > 32).  pcpd_thresholds reports column 0's thresholds. */
+PCPD_API pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, const double *p_w, uint64_t seed,
+                         int variant, uint32_t T_s, uint32_t D, uint32_t A, uint64_t word_offset);
+
 /* mode 0: all sites occupied; 1: i.i.d. Bernoulli(1/2) from the INIT stream
  * (C8: word(i,w) = low 64 bits of block (i, 0, w, 4<<24)); 2: empty.
  * Resets the sweep counter to 0.  Asynchronous. */

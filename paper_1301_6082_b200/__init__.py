@@ -30,7 +30,7 @@ LIB_PATH = os.path.join(_HERE, "libpcpd.so")
 
 # every symbol include/pcpd.h declares
 EXPORTS = (
-    "pcpd_set_allocator", "pcpd_set_stream", "pcpd_create", "pcpd_create_ex", "pcpd_init", "pcpd_run",
+    "pcpd_set_allocator", "pcpd_set_stream", "pcpd_create", "pcpd_create_ex", "pcpd_create_scan", "pcpd_init", "pcpd_run",
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench",
@@ -76,6 +76,9 @@ def load_library() -> C.CDLL:
     L.pcpd_create_ex.argtypes = [C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_uint64, C.c_int,
                                  C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64]
     L.pcpd_create_ex.restype = C.c_void_p
+    L.pcpd_create_scan.argtypes = [C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_uint64, C.c_int,
+                                   C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64]
+    L.pcpd_create_scan.restype = C.c_void_p
     L.pcpd_init.argtypes = [C.c_void_p, C.c_int]
     L.pcpd_init.restype = C.c_int
     L.pcpd_run.argtypes = [C.c_void_p, C.c_uint64]
@@ -163,7 +166,13 @@ class Pcpd:
         _install_torch_allocator(lib)
         self._lib = lib
         torch.cuda.current_stream()  # make sure the context exists
-        if Ts is None and D is None and A is None and word_offset == 0:
+        if np.ndim(d) or np.ndim(p):   # per-word-column probabilities: pcpd_create_scan
+            W = int(n_replicas) // 64
+            dw = np.ascontiguousarray(np.broadcast_to(np.asarray(d, dtype=np.float64), (W,)))
+            pw = np.ascontiguousarray(np.broadcast_to(np.asarray(p, dtype=np.float64), (W,)))
+            h = lib.pcpd_create_scan(L, n_replicas, dw.ctypes.data, pw.ctypes.data, seed, variant, Ts or DEFAULT_TS,
+                                     D or DEFAULT_D, A or DEFAULT_A, word_offset)
+        elif Ts is None and D is None and A is None and word_offset == 0:
             h = lib.pcpd_create(L, n_replicas, d, p, seed, variant)
         else:
             h = lib.pcpd_create_ex(L, n_replicas, d, p, seed, variant, Ts or DEFAULT_TS, D or DEFAULT_D,

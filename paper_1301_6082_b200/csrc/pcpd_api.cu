@@ -79,6 +79,7 @@ struct pcpd_s {
     int Wb;
     uint64_t sweep;
     bool force_block;  // test hook (env PCPD_FORCE_BLOCK_KERNEL=1 at create): run the generic block kernel
+    uint32_t *thr;     // device, per-word thresholds [W][4] (pcpd_create_scan), else NULL
     uint64_t *lat;     // device, word-blocked
     uint32_t *counts;  // device, uint32[R]
     cudaStream_t stream;
@@ -202,6 +203,7 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
                          sweep_smem_bytes(Ts, Wb) <= 200 * 1024;
     }
     h->stream = nullptr;
+    h->thr = nullptr;
     h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
     h->counts = (uint32_t *)dev_alloc(4 * n_replicas, h->stream);
     if (!h->lat || !h->counts) {
@@ -243,10 +245,66 @@ pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_
     return pcpd_create_ex(L, n_replicas, d, p, seed, variant, PCPD_DEFAULT_TS, PCPD_DEFAULT_D, PCPD_DEFAULT_A, 0);
 }
 
+pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, const double *p_w, uint64_t seed,
+                         int variant, uint32_t Ts, uint32_t D, uint32_t A, uint64_t word_offset)
+{
+    if (!d_w || !p_w) {
+        fail(PCPD_ERR_ARG, "create_scan: NULL probability array");
+        return nullptr;
+    }
+    if (variant & PCPD_VARIANT_PMASK_PAPER) {
+        fail(PCPD_ERR_ARG, "create_scan: the paper's annihilation mask is not available with per-word probabilities");
+        return nullptr;
+    }
+    if (n_replicas == 0 || n_replicas % 64) {
+        fail(PCPD_ERR_ARG, "n_replicas must be a positive multiple of 64");
+        return nullptr;
+    }
+    const uint64_t W = n_replicas / 64;
+    for (uint64_t w = 0; w < W; ++w)
+        if (!(d_w[w] >= 0.0 && d_w[w] <= 1.0) || !(p_w[w] >= 0.0 && p_w[w] <= 1.0)) {
+            fail(PCPD_ERR_ARG, "create_scan: d_w[%llu] / p_w[%llu] must lie in [0,1]", (unsigned long long)w,
+                 (unsigned long long)w);
+            return nullptr;
+        }
+    if (Ts == 0 || D == 0 || (uint64_t)((Ts > L ? L : Ts) / D) > 32) {
+        fail(PCPD_ERR_ARG, "create_scan needs at most 32 domains per tile (T_s / D <= 32)");
+        return nullptr;
+    }
+    pcpd_t *h = pcpd_create_ex(L, n_replicas, d_w[0], p_w[0], seed, variant, Ts, D, A, word_offset);
+    if (!h) return nullptr;
+    uint32_t *host = new (std::nothrow) uint32_t[4 * W];
+    h->thr = (uint32_t *)dev_alloc(16 * W, h->stream);
+    if (!host || !h->thr) {
+        delete[] host;
+        pcpd_destroy(h);
+        fail(PCPD_ERR_ALLOC, "create_scan: allocation of the threshold table failed");
+        return nullptr;
+    }
+    for (uint64_t w = 0; w < W; ++w) {
+        const uint64_t Td = threshold_of(d_w[w]), Tp = threshold_of(p_w[w]);
+        host[4 * w + 0] = (Td >> 32) ? 0u : (uint32_t)Td;
+        host[4 * w + 1] = (Tp >> 32) ? 0u : (uint32_t)Tp;
+        host[4 * w + 2] = ((Td >> 32) ? 1u : 0u) | ((Tp >> 32) ? 2u : 0u);
+        host[4 * w + 3] = 0u;
+    }
+    const cudaError_t e = cudaMemcpy(h->thr, host, 16 * W, cudaMemcpyHostToDevice);
+    delete[] host;
+    if (e != cudaSuccess) {
+        pcpd_destroy(h);
+        cuda_fail(e, "create_scan: upload of the threshold table");
+        return nullptr;
+    }
+    h->P.thr_dev = h->thr;
+    h->force_block = false;
+    return h;
+}
+
 void pcpd_destroy(pcpd_t *h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
+    dev_free(h->thr);
     dev_free(h->lat);
     dev_free(h->counts);
     delete h;

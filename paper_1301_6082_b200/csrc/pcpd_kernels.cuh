@@ -35,6 +35,9 @@ struct SweepParams {
     // (tb_(-1) = tb_32 = 0); stopping after M blocks closes the sum with cl[M] = -tb_(2M-1).
     int32_t sd[34], sp[34];
     int32_t cld[18], clp[18];
+    // Per-word-column thresholds (C11, pcpd_create_scan): device array [W][4] = {T_d low 32 bits, T_p low 32 bits,
+    // flags (bit 0: T_d = 2^32, bit 1: T_p = 2^32), 0}; NULL in the uniform mode.
+    const uint32_t *thr_dev;
     uint32_t connected;       // 1: connected multispin lattice: words of tile sites past the ring wrap are bit-rotated (C10)
     uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
 };

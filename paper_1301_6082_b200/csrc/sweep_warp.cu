@@ -178,7 +178,7 @@ __device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &b
 // parameters so that the unconditional part has no branch at all): 5 and 4 for thresholds with that
 // many blocks (tuned on B200: a warp pays the maximum over its 32 lanes, so nearly every attempt
 // needs that many anyway), 1 for thresholds with few planes (d = 1/2 has one), 0 for T = 0 or 2^32.
-template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE>
+template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
@@ -243,8 +243,32 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     const bool act = lane < n;
     const uint32_t b = act ? lane : 0u;
     const uint32_t slot0 = (tau * n + b) * D;
-    const uint32_t nblkD = (P.thd.nplanes + 1u) >> 1, nblkP = (P.thp.nplanes + 1u) >> 1;
-    const uint32_t Td = P.thd.T32, Tp = P.thp.T32;
+    uint32_t nblkD = (P.thd.nplanes + 1u) >> 1, nblkP = (P.thp.nplanes + 1u) >> 1;
+    uint32_t Td = P.thd.T32, Tp = P.thp.T32;
+    bool allD = P.thd.all != 0, allP = P.thp.all != 0;
+    // Per-word thresholds (C11): the bit masks and signed-sum coefficients of the unconditional planes live in
+    // registers for the whole task instead of the constant bank.  Planes past a word's last significant one have
+    // T bit 0, which closes the signed sum at the right plane by itself.
+    uint32_t tdm_r[2 * NU_D + 1], tpm_r[2 * NU_P + 1];
+    int32_t sd_r[2 * NU_D + 1], sp_r[2 * NU_P + 1];
+    if constexpr (PW) {
+        const uint4 th = reinterpret_cast<const uint4 *>(P.thr_dev)[wl];
+        Td = th.x; Tp = th.y; allD = (th.z & 1u) != 0; allP = (th.z & 2u) != 0;
+        nblkD = Td ? (32u - (uint32_t)(__ffs((int)Td) - 1) + 1u) >> 1 : 0u;
+        nblkP = Tp ? (32u - (uint32_t)(__ffs((int)Tp) - 1) + 1u) >> 1 : 0u;
+#pragma unroll
+        for (int kk = 0; kk < 2 * NU_D; ++kk) {
+            const uint32_t bit = (Td >> (31 - kk)) & 1u, prev = kk ? (Td >> (32 - kk)) & 1u : 0u;
+            tdm_r[kk] = 0u - bit;
+            sd_r[kk] = (int32_t)bit - (int32_t)prev;
+        }
+#pragma unroll
+        for (int kk = 0; kk < 2 * NU_P; ++kk) {
+            const uint32_t bit = (Tp >> (31 - kk)) & 1u, prev = kk ? (Tp >> (32 - kk)) & 1u : 0u;
+            tpm_r[kk] = 0u - bit;
+            sp_r[kk] = (int32_t)bit - (int32_t)prev;
+        }
+    }
 
     for (uint32_t k = 0; k < S; ++k) {
         if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, P.rk).x0, D);
@@ -298,11 +322,14 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
 #pragma unroll
             for (int m = 0; m < NU_D; ++m)
-                cmp_block_sum(dlt, dund, dblk[m], P.tdm[2 * m], P.tdm[2 * m + 1], P.sd[2 * m], P.sd[2 * m + 1]);
+                cmp_block_sum(dlt, dund, dblk[m], PW ? tdm_r[2 * m] : P.tdm[2 * m], PW ? tdm_r[2 * m + 1] : P.tdm[2 * m + 1],
+                              PW ? sd_r[2 * m] : P.sd[2 * m], PW ? sd_r[2 * m + 1] : P.sd[2 * m + 1]);
             if constexpr (PMODE == 0) {
 #pragma unroll
                 for (int m = 0; m < NU_P; ++m)
-                    cmp_block_sum(plt, pund, pblk[m], P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m], P.sp[2 * m + 1]);
+                    cmp_block_sum(plt, pund, pblk[m], PW ? tpm_r[2 * m] : P.tpm[2 * m],
+                                  PW ? tpm_r[2 * m + 1] : P.tpm[2 * m + 1], PW ? sp_r[2 * m] : P.sp[2 * m],
+                                  PW ? sp_r[2 * m + 1] : P.sp[2 * m + 1]);
             }
             {
                 const uint64_t rel = sb | sc;
@@ -310,17 +337,25 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 dund.hi &= (uint32_t)(rel >> 32);
                 uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top (0 past the last plane)
                 uint32_t m = NU_D;
+                int32_t prev = NU_D > 0 ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;  // T's bit of the last plane done (PW)
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, P.rk);
-                    cmp_block_sum(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31),
-                                  P.sd[2 * m], P.sd[2 * m + 1]);
+                    int32_t s0, s1;
+                    if constexpr (PW) {
+                        const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
+                        s0 = b0 - prev; s1 = b1 - b0; prev = b1;
+                    } else {
+                        s0 = P.sd[2 * m]; s1 = P.sd[2 * m + 1];
+                    }
+                    cmp_block_sum(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31), s0, s1);
                     Tsh <<= 2;
                 }
                 // close the sum: lanes still equal to T after the last plane looked at are not < T
-                dlt.lo += dund.lo * (uint32_t)P.cld[m];
-                dlt.hi += dund.hi * (uint32_t)P.cld[m];
+                const uint32_t cl = PW ? (uint32_t)(-prev) : (uint32_t)P.cld[m];
+                dlt.lo += dund.lo * cl;
+                dlt.hi += dund.hi * cl;
             }
-            const uint64_t Dm = P.thd.all ? ~0ull : m64(dlt);
+            const uint64_t Dm = allD ? ~0ull : m64(dlt);
             uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
             if constexpr (VARIANT >= 1) react &= se;
             if constexpr (VARIANT >= 2) react &= sf;
@@ -329,14 +364,22 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 pund.hi &= (uint32_t)(react >> 32);
                 uint32_t Tsh = Tp << (2 * NU_P);
                 uint32_t m = NU_P;
+                int32_t prev = NU_P > 0 ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, P.rk);
-                    cmp_block_sum(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31),
-                                  P.sp[2 * m], P.sp[2 * m + 1]);
+                    int32_t s0, s1;
+                    if constexpr (PW) {
+                        const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
+                        s0 = b0 - prev; s1 = b1 - b0; prev = b1;
+                    } else {
+                        s0 = P.sp[2 * m]; s1 = P.sp[2 * m + 1];
+                    }
+                    cmp_block_sum(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31), s0, s1);
                     Tsh <<= 2;
                 }
-                plt.lo += pund.lo * (uint32_t)P.clp[m];
-                plt.hi += pund.hi * (uint32_t)P.clp[m];
+                const uint32_t cl = PW ? (uint32_t)(-prev) : (uint32_t)P.clp[m];
+                plt.lo += pund.lo * cl;
+                plt.hi += pund.hi * cl;
             } else {
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
                 // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
@@ -345,7 +388,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
                 plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
             }
-            const uint64_t Pm = (PMODE == 0 && P.thp.all) ? ~0ull : m64(plt);
+            const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);
 
             // C6 / Alg. 2, branch-free over the 64 replicas.
             uint64_t nb = (Dm & sc) | (~Dm & sb);
@@ -436,15 +479,15 @@ int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks)
 static int nu_d_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUD_BIG ? 1 : PCPD_NUD_BIG; }
 static int nu_p_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < PCPD_NUP_BIG ? 1 : PCPD_NUP_BIG; }
 
-template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE>
+template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW = 0>
 static int warp_op(const SweepParams *P, cudaStream_t stream)
 {
     if (!P)  // configure
-        return (int)cudaFuncSetAttribute(sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE>,
+        return (int)cudaFuncSetAttribute(sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE, PW>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          WPB >= 4 ? 116 * 1024 : 226 * 1024);
     const uint32_t ntasks = (P->L / P->Ts) * P->W;
-    sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE>
+    sweep_warp_kernel<VARIANT, WPB, NU_D, NU_P, PMODE, PW>
         <<<(ntasks + WPB - 1) / WPB, WPB * 32, warp_smem_bytes(P->Ts, WPB), stream>>>(*P);
     return 1;
 }
@@ -452,6 +495,7 @@ static int warp_op(const SweepParams *P, cudaStream_t stream)
 template <int VARIANT, int WPB, int NU_D>
 static int warp_op_p(int nup, const SweepParams *P, cudaStream_t stream)
 {
+    if (nup == -2) return warp_op<VARIANT, WPB, PCPD_NUD_BIG, PCPD_NUP_BIG, 0, 1>(P, stream);  // per-word thresholds
     if (nup == -1) return warp_op<VARIANT, WPB, NU_D, 1, 1>(P, stream);  // paper annihilation mask: ANNI block 0 only
     if (nup == 0) return warp_op<VARIANT, WPB, NU_D, 0, 0>(P, stream);
     if (nup == 1) return warp_op<VARIANT, WPB, NU_D, 1, 0>(P, stream);
@@ -477,6 +521,7 @@ static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams
 
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
 {
+    if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
     return warp_op_any(variant, wpb, nu_d_of((P.thd.nplanes + 1) >> 1), nup, &P, stream);
 }
@@ -485,12 +530,15 @@ int configure_warp_kernels()
 {
     const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[4] = {-1, 0, 1, PCPD_NUP_BIG}, wpbs[2] = {7, 1};
     for (int variant = 0; variant < 3; ++variant)
-        for (int wpb : wpbs)
+        for (int wpb : wpbs) {
             for (int nud : nuds)
                 for (int nup : nups) {
                     const int e = warp_op_any(variant, wpb, nud, nup, nullptr, nullptr);
                     if (e != 0) return e;
                 }
+            const int e = warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, nullptr, nullptr);
+            if (e != 0) return e;
+        }
     return 0;
 }
 

@@ -339,3 +339,36 @@ def test_long_parity_protocol(pk, name, words, times):
     if times == "all":
         times = [t for t in wl.record_times(c.sweeps) if t > 0]
     gpu_check(pk, kw, {}, c.init, times, words=words)
+
+
+def test_per_word_probabilities_scan(pk):
+    """pcpd_create_scan (contract C11, next-row f4): every word column has its own (d, p); bit-exact against the
+    oracle in the same mode, and column k equals the uniform GPU run with (d_k, p_k)."""
+    L, W = 4096, 6
+    ds = np.array([0.8, 0.5, 0.1, 1.0, 0.0, 0.3])
+    ps = np.array([0.12, 0.152, 0.09, 0.3, 0.2, 0.0])
+    for variant in (pk.PCPD, pk.TCPD | pk.CONNECTED):
+        g = pk.Pcpd(L, 64 * W, ds, ps, 41, variant)
+        o = oracle.Oracle(L, 64 * W, 0.25, 0.25, 41, variant)
+        for k in range(W):
+            o.set_word_probabilities(k, ds[k], ps[k])
+        g.init(pk.INIT_BERNOULLI)
+        o.init(1)
+        for _ in range(4):
+            g.run(2)
+            o.run(2)
+            assert np.array_equal(g.get_lattice(), o.get_words())
+            assert np.array_equal(g.density(), o.counts())
+        lat = g.get_lattice()
+        g.close()
+        if variant == pk.PCPD:
+            for k in (0, 3):
+                u = pk.Pcpd(L, 64, float(ds[k]), float(ps[k]), 41, variant, word_offset=k)
+                u.init(pk.INIT_BERNOULLI)
+                u.run(8)
+                assert np.array_equal(u.get_lattice()[:, 0], lat[:, k])
+                u.close()
+    with pytest.raises(pk.PcpdError):
+        pk.Pcpd(L, 64 * W, ds, ps, 41, pk.PCPD | pk.PMASK_PAPER)
+    with pytest.raises(pk.PcpdError):
+        pk.Pcpd(L, 64 * W, ds + 0.5, ps, 41, pk.PCPD)
