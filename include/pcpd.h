@@ -96,7 +96,7 @@ PCPD_API int pcpd_set_stream(pcpd_t *h, void *cuda_stream);
  * pcpd_create: variant 0 = PCPD, 1 = TCPD.  Schedule SD2(2048, 64, 4).
  * Errors (NULL): n_replicas == 0 or not a multiple of 64; L not a multiple of
  * the domain length D, or L < D; T_s is clamped to L when L < T_s, otherwise
- * L % T_s != 0 is an error; d, p outside [0,1] or NaN; L >= 2^32 or
+ * L % T_s != 0 is an error; d, p outside [0,1] or NaN; L > 2^31 or
  * W >= 2^32; unknown variant; allocation failure; no sm_100 device. */
 PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p, uint64_t seed, int variant);
 

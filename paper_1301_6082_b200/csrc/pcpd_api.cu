@@ -123,8 +123,8 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_ARG, "the paper's annihilation mask needs p < 1/4");
         return nullptr;
     }
-    if (L == 0 || L >= (1ull << 32) || word_offset + W >= (1ull << 32)) {
-        fail(PCPD_ERR_ARG, "L and word_offset + W must be < 2^32 (32-bit counter fields)");
+    if (L == 0 || L > (1ull << 31) || word_offset + W >= (1ull << 32)) {
+        fail(PCPD_ERR_ARG, "L must be <= 2^31 and word_offset + W < 2^32 (32-bit counter fields and site indices)");
         return nullptr;
     }
     if (D == 0 || A == 0 || Ts == 0 || D % A) {

@@ -117,6 +117,7 @@ SMALL = [
     (2, 4096, 128, 0.5, 0.03, 2048, 64, 4, 0),       # QCPD, 6-site footprint
     (2, 1408, 128, 0.3, 0.1, 704, 11, 1, 1),         # QCPD, smallest legal domain D = 11 (n = 64: block kernel)
     (0x102, 2048, 64, 0.25, 0.05, 1024, 32, 2, 1),   # QCPD with the paper's annihilation mask
+    (0, 2048, 64, 0.3, 0.12, 2048, 64, 1, 1),        # A = 1: S = 64 sub-steps (more than one group of 32 shifts per sweep)
     (0x200, 4096, 256, 0.3, 0.12, 2048, 64, 4, 1),   # the paper's connected multispin lattice (bit rotation at the ring wrap)
     (0x200, 1024, 64, 0.5, 0.15, 2048, 64, 4, 0),    # same, single tile = whole ring (T_s clamped to L)
     (0x300, 147, 64, 0.37, 0.21, 49, 7, 1, 1),       # same + paper mask, odd L and T_s (64-bit tile copy path)
