@@ -231,13 +231,31 @@ void oracle_rule_qcpd(uint8_t *qm1, uint8_t *q0, uint8_t *q1, uint8_t *q2, uint8
     }
 }
 
+/* CPD, the contact process with diffusion: the one-particle member of the family PCPD (pairs),
+ * TCPD (triples), QCPD (quadruplets), which is in the directed-percolation class - this build's
+ * reading of the "DP" model the paper says the algorithm extends to (it prints no
+ * rule; next-row f4 of SURVEY.md 8(f)).  By the same analogy with Alg. 1: A0/0A -> AA each at rate
+ * (1-p)(1-d)/2, A -> 0 at rate p(1-d), A0 <-> 0A at rate d; footprint {x-1, x, x+1}; diffusion
+ * swaps (x, x+1); the fission-high target x+1 is the swap partner's site. */
+void oracle_rule_cpd(uint8_t *qm1, uint8_t *q0, uint8_t *q1, int Dm, int Pm, int Fm)
+{
+    if (Dm) {
+        uint8_t tmp = *q0; *q0 = *q1; *q1 = tmp;
+    } else if (*q0 == 1) {
+        if (Pm) { *q0 = 0; }
+        else if (Fm) { *qm1 = 1; }
+        else { *q1 = 1; }
+    }
+}
+
 /* Single attempt on a periodic ring of L sites at site i (literal indexing,
  * reading G2: indices mod L).  Exposed for the master-equation pin P4. */
 void oracle_single_attempt(int variant, uint32_t L, uint8_t *q, uint32_t i,
                            int Dm, int Pm, int Fm)
 {
     uint32_t im1 = (i + L - 1) % L, i1 = (i + 1) % L, i2 = (i + 2) % L, i3 = (i + 3) % L, i4 = (i + 4) % L;
-    if (variant == 0)      oracle_rule_pcpd(&q[im1], &q[i], &q[i1], &q[i2], Dm, Pm, Fm);
+    if (variant == 3)      oracle_rule_cpd(&q[im1], &q[i], &q[i1], Dm, Pm, Fm);
+    else if (variant == 0) oracle_rule_pcpd(&q[im1], &q[i], &q[i1], &q[i2], Dm, Pm, Fm);
     else if (variant == 1) oracle_rule_tcpd(&q[im1], &q[i], &q[i1], &q[i2], &q[i3], Dm, Pm, Fm);
     else                   oracle_rule_qcpd(&q[im1], &q[i], &q[i1], &q[i2], &q[i3], &q[i4], Dm, Pm, Fm);
 }
@@ -245,7 +263,7 @@ void oracle_single_attempt(int variant, uint32_t L, uint8_t *q, uint32_t i,
 /* --------------------------------------------------------------- handle --- */
 typedef struct oracle_t {
     uint32_t L, Ts, D, A;
-    int variant;               /* 0 PCPD, 1 TCPD, 2 QCPD */
+    int variant;               /* 0 PCPD, 1 TCPD, 2 QCPD, 3 CPD (contact process with diffusion) */
     int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
     int connected;             /* 1: the paper's connected multispin lattice (C10, below) */
     uint64_t Td, Tp, T4p;
@@ -274,9 +292,9 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     /* | ORACLE_CONNECTED (0x200): the paper's connected multispin lattice, C10. */
     int connected = (variant & 0x200) ? 1 : 0;
     variant &= ~0x300;
-    if (variant != 0 && variant != 1 && variant != 2) return NULL;
+    if (variant < 0 || variant > 3) return NULL;
     if (pmask_paper && !(p < 0.25)) return NULL;
-    uint32_t Rr = 2u + (uint32_t)variant;      /* right reach: 2 PCPD, 3 TCPD, 4 QCPD */
+    uint32_t Rr = variant == 3 ? 1u : 2u + (uint32_t)variant;   /* right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD */
     if (L == 0 || L >= ((uint64_t)1 << 32) || nwords == 0) return NULL;
     if (Ts > L) Ts = (uint32_t)L;
     if (D == 0 || A == 0 || Ts == 0) return NULL;
@@ -371,7 +389,7 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
 {
     const uint32_t L = o->L, Ts = o->Ts, D = o->D;
     const uint32_t n = Ts / D;
-    const uint32_t Rr = 2u + (uint32_t)o->variant;
+    const uint32_t Rr = o->variant == 3 ? 1u : 2u + (uint32_t)o->variant;
     const uint32_t w = o->words[k];
 
     /* C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
@@ -431,7 +449,9 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
         /* Fm = mask(1/2) from plane `lo` (C4): U_j < 2^31 <=> top bit of U_j,
          * i.e. lane j of plane 0, is 0.  Fm = 1 => fission LOW (G8). */
         int Fm = ((misc_lo >> j) & 1u) == 0 ? 1 : 0;
-        if (o->variant == 0)
+        if (o->variant == 3)
+            oracle_rule_cpd(qs[0], qs[1], qs[2], Dm[j], Pm[j], Fm);
+        else if (o->variant == 0)
             oracle_rule_pcpd(qs[0], qs[1], qs[2], qs[3], Dm[j], Pm[j], Fm);
         else if (o->variant == 1)
             oracle_rule_tcpd(qs[0], qs[1], qs[2], qs[3], qs[4], Dm[j], Pm[j], Fm);
@@ -551,7 +571,7 @@ int oracle_literal_run(int variant, uint32_t L, uint32_t R, double d, double p,
 {
     uint64_t Td = oracle_threshold(d), Tp = oracle_threshold(p);
     if (Td == UINT64_MAX || Tp == UINT64_MAX) return -1;
-    if (variant < 0 || variant > 2 || L < 4u + (uint32_t)variant) return -1;      /* reading G18 */
+    if (variant < 0 || variant > 3 || L < (variant == 3 ? 3u : 4u + (uint32_t)variant)) return -1;  /* reading G18 */
     uint32_t t = 0;
     for (uint32_t rec = 0; rec < n_rec; ++rec) {
         for (; t < rec_times[rec]; ++t)

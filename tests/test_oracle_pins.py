@@ -120,7 +120,7 @@ def test_P0p_streams_and_words_are_distinct():
 SCHEDULES = [dict(Ts=2048, D=64, A=4), dict(Ts=64, D=64, A=64), dict(Ts=32, D=16, A=2)]
 
 
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD, wl.CPD])
 @pytest.mark.parametrize("sch", SCHEDULES)
 def test_P1_empty_lattice_is_absorbing(variant, sch):
     o = oracle.Oracle(128, 128, 0.3, 0.2, 11, variant, **sch)
@@ -129,7 +129,7 @@ def test_P1_empty_lattice_is_absorbing(variant, sch):
     assert not o.get_words().any() and not o.counts().any()
 
 
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD, wl.CPD])
 @pytest.mark.parametrize("sch", SCHEDULES)
 def test_P2_d_equals_one_conserves_particles(variant, sch):
     o = oracle.Oracle(128, 128, 1.0, 0.3, 12, variant, **sch)
@@ -197,7 +197,7 @@ def master_matrix(variant, L, d, p):
     outer neighbour at (1-p)(1-d)/2; diagonal by normalisation."""
     n = 1 << L
     P = [[Fraction(0)] * n for _ in range(n)]
-    k = 2 + variant  # cluster size: 2 PCPD, 3 TCPD, 4 QCPD
+    k = 1 if variant == wl.CPD else 2 + variant  # cluster size: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
     for s in range(n):
         b = _bits(s, L)
         for i in range(L):
@@ -237,7 +237,7 @@ def oracle_matrix(variant, L, d, p):
 
 
 @pytest.mark.parametrize("variant,L", [(wl.PCPD, 4), (wl.PCPD, 5), (wl.PCPD, 6), (wl.TCPD, 5), (wl.TCPD, 6),
-                                       (wl.QCPD, 6), (wl.QCPD, 7)])
+                                       (wl.QCPD, 6), (wl.QCPD, 7), (wl.CPD, 3), (wl.CPD, 4), (wl.CPD, 5)])
 def test_P4_master_equation_enumeration(variant, L):
     d, p = Fraction(3, 10), Fraction(7, 40)
     assert master_matrix(variant, L, d, p) == oracle_matrix(variant, L, d, p)  # exact rationals
@@ -257,7 +257,7 @@ def test_P4_fission_side_follows_alg1():
     assert list(oracle.single_attempt(wl.PCPD, [1, 0, 0, 0, 0, 1], 5, 0, 0, 0)) == [1, 1, 0, 0, 0, 1]
 
 
-@pytest.mark.parametrize("variant,L", [(wl.PCPD, 6), (wl.TCPD, 6), (wl.QCPD, 6)])
+@pytest.mark.parametrize("variant,L", [(wl.PCPD, 6), (wl.TCPD, 6), (wl.QCPD, 6), (wl.CPD, 5)])
 def test_P4_literal_mode_mean_density_vs_master_equation(variant, L):
     """E[count] after n = 1, 2, 3 time units (n*L attempts) from P^(nL) (floats
     from the exact-rational matrix) vs the literal Alg. 1 Monte Carlo mean."""
@@ -279,7 +279,7 @@ def test_P4_literal_mode_mean_density_vs_master_equation(variant, L):
 
 
 # ------------------------------------------------------------------ P7 ----
-@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD])
+@pytest.mark.parametrize("variant", [wl.PCPD, wl.TCPD, wl.QCPD, wl.CPD])
 def test_P7_run_splitting_loop_order_word_subsets(variant):
     kw = dict(L=256, n_replicas=256, d=0.3, p=0.12, seed=21, variant=variant, Ts=128, D=32, A=4)
     a = oracle.Oracle(**kw)
