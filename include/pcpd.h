@@ -55,7 +55,10 @@ enum pcpd_status {
 /* 0 PCPD (eq. (1)); 1 TCPD (config 5: triples, 5-site footprint); 2 QCPD (quadruplets
  * AAAA0/0AAAA -> AAAAA at (1-p)(1-d)/2 each, AAAA -> 0000 at p(1-d), A0 <-> 0A at d; 6-site footprint
  * {x-1 .. x+4}; needs D >= 11). */
-enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1, PCPD_VARIANT_QCPD = 2 };
+/* 3 CPD: the contact process with diffusion, the one-particle member of that family (directed-percolation
+ * class; this build's reading of the "DP" model of PAPER.md:15, 21): A0/0A -> AA at (1-p)(1-d)/2 each, A -> 0 at
+ * p(1-d), A0 <-> 0A at d; 3-site footprint {x-1, x, x+1}; needs D >= 5. */
+enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1, PCPD_VARIANT_QCPD = 2, PCPD_VARIANT_CPD = 3 };
 /* Flag to OR into `variant`: use the PAPER's OWN annihilation mask instead of independent
  * per-lane Bernoulli(p) bits (Alg. 2 lines 12-13; section 4.3):
  * lane j of Pm = a0_j & a1_j & [u < 4p], a0/a1 = the two 64-lane planes of ANNI block 0 (an
@@ -105,7 +108,7 @@ PCPD_API pcpd_t *pcpd_create(uint64_t L, uint64_t n_replicas, double d, double p
  * for bit; used by the parity tests to cross-check the two kernels at full size). */
 
 /* Same with explicit schedule constants (D | T_s | L, A | D, D >= 2*Rr+3 with
- * Rr = 2 PCPD / 3 TCPD / 4 QCPD; T_s*8 bytes (one tile column) must fit the 227 KB shared memory) and
+ * Rr = 2 PCPD / 3 TCPD / 4 QCPD / 1 CPD; T_s*8 bytes (one tile column) must fit the 227 KB shared memory) and
  * a global word offset: the handle simulates word columns
  * word_offset .. word_offset + W - 1 of a larger run (multi-GPU sharding by
  * replica words); columns never interact, so the union of

@@ -19,7 +19,7 @@ import numpy as np
 
 from .shard import gather_counts, max_over_ranks, shard_words  # noqa: F401
 
-PCPD, TCPD, QCPD = 0, 1, 2
+PCPD, TCPD, QCPD, CPD = 0, 1, 2, 3
 CONNECTED = 0x200    # OR into `variant`: the paper's connected multispin lattice (PCPD_VARIANT_CONNECTED)
 PMASK_PAPER = 0x100  # OR into `variant`: the paper's own annihilation mask (PCPD_VARIANT_PMASK_PAPER)
 INIT_FULL, INIT_BERNOULLI, INIT_EMPTY = 0, 1, 2

@@ -105,11 +105,12 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     const int pmask_paper = (variant & PCPD_VARIANT_PMASK_PAPER) ? 1 : 0;
     const int connected = (variant & PCPD_VARIANT_CONNECTED) ? 1 : 0;
     variant &= ~(PCPD_VARIANT_PMASK_PAPER | PCPD_VARIANT_CONNECTED);
-    if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD && variant != PCPD_VARIANT_QCPD) {
+    if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD && variant != PCPD_VARIANT_QCPD &&
+        variant != PCPD_VARIANT_CPD) {
         fail(PCPD_ERR_ARG, "unknown variant %d", variant);
         return nullptr;
     }
-    const uint32_t Rr = 2u + (uint32_t)variant;
+    const uint32_t Rr = variant == PCPD_VARIANT_CPD ? 1u : 2u + (uint32_t)variant;
     if (n_replicas == 0 || n_replicas % 64) {
         fail(PCPD_ERR_ARG, "n_replicas must be a positive multiple of 64");
         return nullptr;

@@ -53,7 +53,7 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
     __shared__ uint32_t s_sigma[MAX_SUBSTEPS];
     __shared__ uint32_t s_Sigma;
 
-    constexpr uint32_t Rr = 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD
+    constexpr uint32_t Rr = VARIANT == 3 ? 1u : 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
     const uint32_t tau = blockIdx.x, wg = blockIdx.y;
     const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
@@ -117,16 +117,18 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
             if (y0 >= Ts) y0 -= Ts;
             uint64_t *q = tile + (size_t)y0 * WB + wl;
 
-            uint64_t sa = q[0], sb = q[WB], sc = q[2 * WB], se = q[3 * WB];
-            uint64_t sf = 0, sg = 0;
-            if constexpr (VARIANT >= 1) sf = q[4 * WB];
-            if constexpr (VARIANT >= 2) sg = q[5 * WB];
+            uint64_t sa = q[0], sb = q[WB], sc = q[2 * WB];
+            uint64_t se = 0, sf = 0, sg = 0;
+            if constexpr (VARIANT != 3) se = q[3 * WB];
+            if constexpr (VARIANT == 1 || VARIANT == 2) sf = q[4 * WB];
+            if constexpr (VARIANT == 2) sg = q[5 * WB];
 
             // C6 / Alg. 2, branch-free over the 64 replicas.
             const uint64_t Dm = lazy_mask<STREAM_DIFF>(sb | sc, P.thd, slot, t, w, P.rk);
-            uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
-            if constexpr (VARIANT >= 1) react &= se;
-            if constexpr (VARIANT >= 2) react &= sf;
+            uint64_t react = sb & ~Dm;  // particle cluster present and no diffusion
+            if constexpr (VARIANT != 3) react &= sc;
+            if constexpr (VARIANT == 1 || VARIANT == 2) react &= se;
+            if constexpr (VARIANT == 2) react &= sf;
             const uint64_t Pm = lazy_mask<STREAM_ANNI>(react, P.thp, slot, t, w, P.rk);
             const uint64_t Fm = ~lo64(misc);  // 1 -> fission low (Alg. 1: r3 < 1/2)
             uint64_t nb = (Dm & sc) | (~Dm & sb);
@@ -134,9 +136,11 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
             const uint64_t ann = react & Pm;
             const uint64_t fis = react & ~Pm;
             nb &= ~ann;
-            nc &= ~ann;
+            if constexpr (VARIANT != 3) nc &= ~ann;
             sa |= fis & Fm;
-            if constexpr (VARIANT == 0) {
+            if constexpr (VARIANT == 3) {
+                nc |= fis & ~Fm;
+            } else if constexpr (VARIANT == 0) {
                 se |= fis & ~Fm;
             } else if constexpr (VARIANT == 1) {
                 se &= ~ann;
@@ -152,7 +156,7 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
             q[0] = sa;
             q[WB] = nb;
             q[2 * WB] = nc;
-            q[3 * WB] = se;
+            if constexpr (VARIANT != 3) q[3 * WB] = se;
         }
         __syncthreads();
     }
@@ -194,7 +198,8 @@ int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cud
 {
     if (sweep_warp_supported(P.Ts, P.D) && !force_block_kernel)
         return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream);
-    return variant == 0 ? launch_sweep_t<0>(P, stream) : variant == 1 ? launch_sweep_t<1>(P, stream) : launch_sweep_t<2>(P, stream);
+    return variant == 0 ? launch_sweep_t<0>(P, stream) : variant == 1 ? launch_sweep_t<1>(P, stream)
+           : variant == 2 ? launch_sweep_t<2>(P, stream) : launch_sweep_t<3>(P, stream);
 }
 
 int configure_kernels()
@@ -205,6 +210,8 @@ int configure_kernels()
     if ((e = cudaFuncSetAttribute(sweep_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
     if ((e = cudaFuncSetAttribute(sweep_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+        return (int)e;
+    if ((e = cudaFuncSetAttribute(sweep_kernel<3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
     return configure_warp_kernels();
 }

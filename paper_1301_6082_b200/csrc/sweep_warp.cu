@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
 
-    constexpr uint32_t Rr = 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD
+    constexpr uint32_t Rr = VARIANT == 3 ? 1u : 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
     const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
@@ -311,9 +311,10 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             uint64_t *q = tile + y0;
             uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0, sg = 0;
             if (act) {
-                sa = q[0]; sb = q[1]; sc = q[2]; se = q[3];
-                if constexpr (VARIANT >= 1) sf = q[4];
-                if constexpr (VARIANT >= 2) sg = q[5];
+                sa = q[0]; sb = q[1]; sc = q[2];
+                if constexpr (VARIANT != 3) se = q[3];
+                if constexpr (VARIANT == 1 || VARIANT == 2) sf = q[4];
+                if constexpr (VARIANT == 2) sg = q[5];
             }
 
             // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
@@ -356,9 +357,10 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 dlt.hi += dund.hi * cl;
             }
             const uint64_t Dm = allD ? ~0ull : m64(dlt);
-            uint64_t react = sb & sc & ~Dm;  // pair (triple) present and no diffusion
-            if constexpr (VARIANT >= 1) react &= se;
-            if constexpr (VARIANT >= 2) react &= sf;
+            uint64_t react = sb & ~Dm;  // particle cluster (1, 2, 3 or 4 sites from x) present and no diffusion
+            if constexpr (VARIANT != 3) react &= sc;
+            if constexpr (VARIANT == 1 || VARIANT == 2) react &= se;
+            if constexpr (VARIANT == 2) react &= sf;
             if constexpr (PMODE == 0) {
                 pund.lo &= (uint32_t)react;
                 pund.hi &= (uint32_t)(react >> 32);
@@ -396,10 +398,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             const uint64_t ann = react & Pm;
             const uint64_t fis = react & ~Pm;
             nb &= ~ann;
-            nc &= ~ann;
+            if constexpr (VARIANT != 3) nc &= ~ann;
             sa |= fis & Fm;
             if (act) {
-                if constexpr (VARIANT == 0) {        // PCPD: pair at x, x+1; fission high -> x+2
+                if constexpr (VARIANT == 3) {        // CPD: single particle at x; fission high -> x+1 (react lanes have Dm = 0)
+                    nc |= fis & ~Fm;
+                } else if constexpr (VARIANT == 0) { // PCPD: pair at x, x+1; fission high -> x+2
                     se |= fis & ~Fm;
                 } else if constexpr (VARIANT == 1) { // TCPD: triple x..x+2; high -> x+3
                     se &= ~ann;
@@ -412,7 +416,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                     q[4] = sf;
                     q[5] = sg;
                 }
-                q[0] = sa; q[1] = nb; q[2] = nc; q[3] = se;
+                q[0] = sa; q[1] = nb; q[2] = nc;
+                if constexpr (VARIANT != 3) q[3] = se;
             }
         }
         __syncwarp();
@@ -512,6 +517,8 @@ static int warp_op_d(int nud, int nup, const SweepParams *P, cudaStream_t stream
 
 static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams *P, cudaStream_t stream)
 {
+    if (variant == 3)
+        return wpb == 7 ? warp_op_d<3, 7>(nud, nup, P, stream) : warp_op_d<3, 1>(nud, nup, P, stream);
     if (variant == 2)
         return wpb == 7 ? warp_op_d<2, 7>(nud, nup, P, stream) : warp_op_d<2, 1>(nud, nup, P, stream);
     if (variant == 0)
@@ -529,7 +536,7 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
 int configure_warp_kernels()
 {
     const int nuds[3] = {0, 1, PCPD_NUD_BIG}, nups[4] = {-1, 0, 1, PCPD_NUP_BIG}, wpbs[2] = {7, 1};
-    for (int variant = 0; variant < 3; ++variant)
+    for (int variant = 0; variant < 4; ++variant)
         for (int wpb : wpbs) {
             for (int nud : nuds)
                 for (int nup : nups) {

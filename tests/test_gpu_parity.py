@@ -117,6 +117,9 @@ SMALL = [
     (2, 4096, 128, 0.5, 0.03, 2048, 64, 4, 0),       # QCPD, 6-site footprint
     (2, 1408, 128, 0.3, 0.1, 704, 11, 1, 1),         # QCPD, smallest legal domain D = 11 (n = 64: block kernel)
     (0x102, 2048, 64, 0.25, 0.05, 1024, 32, 2, 1),   # QCPD with the paper's annihilation mask
+    (3, 4096, 128, 0.5, 0.3, 2048, 64, 4, 0),        # CPD (contact process with diffusion, DP class), 3-site footprint
+    (3, 640, 64, 0.2, 0.4, 320, 5, 1, 1),            # CPD, smallest legal domain D = 5 (n = 64: block kernel)
+    (0x203, 2048, 64, 0.25, 0.2, 1024, 32, 2, 1),    # CPD on the connected lattice
     (0, 2048, 64, 0.3, 0.12, 2048, 64, 1, 1),        # A = 1: S = 64 sub-steps (more than one group of 32 shifts per sweep)
     (0x200, 4096, 256, 0.3, 0.12, 2048, 64, 4, 1),   # the paper's connected multispin lattice (bit rotation at the ring wrap)
     (0x200, 1024, 64, 0.5, 0.15, 2048, 64, 4, 0),    # same, single tile = whole ring (T_s clamped to L)
