@@ -275,3 +275,11 @@ def test_P5_high_statistics_bias_of_the_default_schedule():
     print("  +/- =", np.round(err, 5))
     print("  z   =", np.round(z, 2))
     assert np.all(np.abs(z) < 4.0) and np.all(np.abs(rel) < 0.005), (z, rel)
+
+
+@pytest.mark.slow
+def test_P5_cpd_sd2_matches_literal():
+    times = [1, 2, 4, 8, 16, 32]
+    z, rel, _, _ = _sd2_vs_literal(wl.CPD, 512, 1024, 0.5, 0.3, times, dict(Ts=2048, D=64, A=4))
+    print("P5 cpd z =", np.round(z, 2), "rel =", np.round(rel, 4))
+    assert np.all(np.abs(z) < 4.0), (z, rel)
