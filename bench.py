@@ -331,7 +331,13 @@ def ours_arm(args, cfg: wl.Config) -> None:
                                 f"({mix_peak / 148 / (peaks['sm_max_mhz'] * 1e6):.1f} lanes/clk/SM); nominal issue peak "
                                 f"148 SMs x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz = {nominal_peak / 1e12:.1f} Tinstr/s",
                     hbm=dict(achieved=hbm_bytes / (sweep_ms * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                             frac=hbm_bytes / (sweep_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], peak_source=peaks["source"]))
+                             frac=hbm_bytes / (sweep_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], peak_source=peaks["source"]),
+                    # the other kernel of the step: positional popcount, reads the lattice once (HBM-bound);
+                    # density_ms includes the memset of the counts, their D2H copy and the stream synchronisation
+                    density=dict(bound="hbm", achieved=cfg.lattice_bytes / (density_ms * 1e-3) / 1e9,
+                                 peak=peaks["hbm_gbs"], unit="GB/s",
+                                 frac=cfg.lattice_bytes / (density_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                 call_ms=density_ms))
         cores = max(1, min(os.cpu_count() or 1, cfg.W, 16))
         L_sample = min(cfg.L, 1 << 17)
         _, dt1 = oracle_sample_rate(cfg, L_sample, cores, 1)         # calibration sweep
