@@ -323,7 +323,9 @@ def ours_arm(args, cfg: wl.Config) -> None:
         hbm_bytes = 2.0 * cfg.lattice_bytes
         roof = dict(bound="alu", achieved=achieved / 1e12, peak=mix_peak / 1e12, unit="Tinstr/s",
                     frac=achieved / mix_peak, traffic=NCU_TRAFFIC_BYTES.get(cfg.name),
-                    kernel="sweep_warp_kernel", launch_ms=sweep_ms,
+                    kernel="sweep_warp_kernel" + (" (run-time specialised on T_d, T_p: csrc/jit.cu)" if h.jit_state() == 1
+                                                  else " (built-in generic-threshold kernel)"),
+                    launch_ms=sweep_ms,
                     instr_per_attempt_word=alg["lazy"], lazy_blocks=alg["lazy_blocks"],
                     frac_eager=alg["eager"] * attempt_words / (sweep_ms * 1e-3) / mix_peak,
                     frac_of_nominal_issue=achieved / nominal_peak,

@@ -161,6 +161,27 @@ PCPD_API int pcpd_synchronize(pcpd_t *h);                /* cudaStreamSynchroniz
 PCPD_API void pcpd_destroy(pcpd_t *h);                   /* NULL-safe                  */
 PCPD_API const char *pcpd_last_error(void);              /* thread-local, library-owned */
 
+/* ---- run-time specialisation of the sweep kernel -------
+ * d and p are constants for the life of a handle, and the kernel's compare of the random planes with
+ * the bits of T_d, T_p (C3) is cheaper when those bits are compile-time constants.  For large problems
+ * (at least 148 x 14 tile columns) the first pcpd_run of a handle therefore compiles the SAME device
+ * source with T_d, T_p as template constants (NVRTC, sm_100a; about a second, once per process, device
+ * and parameter set) and runs that kernel from then on.  Results are identical bit for bit.  If
+ * libnvrtc cannot be loaded or the compilation fails, the handle keeps the built-in generic-threshold
+ * CUDA kernel (this is not a CPU fallback) and pcpd_jit_message() says why.  Environment, read by
+ * pcpd_create*: PCPD_JIT=0 never specialise; PCPD_JIT=force specialise at every problem size (test
+ * hook); PCPD_NVRTC_PATH = full path of libnvrtc.so.12 if it is not on the loader path.  Not used with
+ * per-word-column probabilities (pcpd_create_scan), nor when d = 1 or p = 1.
+ * pcpd_jit_state: 1 the handle's sweeps run the specialised kernel; 0 not tried (no sweep yet) or not
+ * applicable; -1 tried and unavailable.  pcpd_jit_launch_count: specialised-kernel launches of this
+ * process (also counted by pcpd_launch_count).  pcpd_jit_selftest: compile only - needs libnvrtc but no
+ * device - sweep_warp_kernel<variant, ..., T_d, T_p> and return the cubin size; PCPD_ERR_DEVICE and the
+ * compiler's message in pcpd_last_error() on failure. */
+PCPD_API int pcpd_jit_state(const pcpd_t *h);
+PCPD_API const char *pcpd_jit_message(void);
+PCPD_API uint64_t pcpd_jit_launch_count(void);
+PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_bytes);
+
 /* Number of kernels this library has launched so far in this process. */
 PCPD_API uint64_t pcpd_launch_count(void);
 

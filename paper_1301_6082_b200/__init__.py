@@ -33,7 +33,8 @@ EXPORTS = (
     "pcpd_set_allocator", "pcpd_set_stream", "pcpd_create", "pcpd_create_ex", "pcpd_create_scan", "pcpd_init", "pcpd_run",
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
-    "pcpd_launch_count", "pcpd_microbench",
+    "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
+    "pcpd_jit_selftest",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -109,6 +110,14 @@ def load_library() -> C.CDLL:
     L.pcpd_launch_count.restype = C.c_uint64
     L.pcpd_microbench.argtypes = [C.c_int, C.c_uint32, C.POINTER(C.c_double)]
     L.pcpd_microbench.restype = C.c_int
+    L.pcpd_jit_state.argtypes = [C.c_void_p]
+    L.pcpd_jit_state.restype = C.c_int
+    L.pcpd_jit_message.argtypes = []
+    L.pcpd_jit_message.restype = C.c_char_p
+    L.pcpd_jit_launch_count.argtypes = []
+    L.pcpd_jit_launch_count.restype = C.c_uint64
+    L.pcpd_jit_selftest.argtypes = [C.c_int, C.c_uint32, C.c_uint32, u64p]
+    L.pcpd_jit_selftest.restype = C.c_int
     _lib = L
     return L
 
@@ -145,6 +154,22 @@ def _check(L, rc):
 
 def launch_count() -> int:
     return int(load_library().pcpd_launch_count())
+
+
+def jit_launch_count() -> int:
+    return int(load_library().pcpd_jit_launch_count())
+
+
+def jit_message() -> str:
+    return (load_library().pcpd_jit_message() or b"").decode()
+
+
+def jit_selftest(variant: int, T_d: int, T_p: int) -> int:
+    """Compile (NVRTC, no device needed) the sweep kernel specialised on the thresholds; returns the cubin size."""
+    L = load_library()
+    n = C.c_uint64(0)
+    _check(L, L.pcpd_jit_selftest(int(variant), int(T_d), int(T_p), C.byref(n)))
+    return int(n.value)
 
 
 def microbench(kind: int, iters: int = 2000) -> float:
@@ -255,6 +280,10 @@ class Pcpd:
     @sweep.setter
     def sweep(self, t):
         _check(self._lib, self._lib.pcpd_set_sweep(self._h, t))
+
+    def jit_state(self) -> int:
+        """1: sweeps run the threshold-specialised kernel; 0: not tried / not applicable; -1: unavailable."""
+        return int(self._lib.pcpd_jit_state(self._h))
 
     def synchronize(self):
         _check(self._lib, self._lib.pcpd_synchronize(self._h))

@@ -84,6 +84,7 @@ struct pcpd_s {
     uint32_t *counts;  // device, uint32[R]
     cudaStream_t stream;
     SweepParams P;
+    JitSlot jit;       // threshold-specialised sweep kernel (jit.cu); mode from env PCPD_JIT at create
 };
 
 extern "C" {
@@ -202,6 +203,12 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         const char *fb = getenv("PCPD_FORCE_BLOCK_KERNEL");
         h->force_block = fb && fb[0] == '1' && !pmask_paper && (uint64_t)(Ts / D) <= 1024 &&
                          sweep_smem_bytes(Ts, Wb) <= 200 * 1024;
+    }
+    {
+        const char *jm = getenv("PCPD_JIT");  // unset / "1": auto (large problems); "0": off; "force": every size
+        h->jit.mode = !jm ? 1 : !strcmp(jm, "0") ? 0 : !strcmp(jm, "force") ? 2 : 1;
+        h->jit.state = 0;
+        h->jit.kernel = nullptr;
     }
     h->stream = nullptr;
     h->thr = nullptr;
@@ -341,7 +348,7 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream);
+        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit);
         h->sweep += 1;
     }
     return check_launch("sweep kernel");
@@ -437,6 +444,19 @@ int pcpd_synchronize(pcpd_t *h)
     if (!h) return fail(PCPD_ERR_ARG, "null handle");
     const cudaError_t e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(e, "synchronize");
+    return PCPD_OK;
+}
+
+int pcpd_jit_state(const pcpd_t *h) { return h ? h->jit.state : 0; }
+const char *pcpd_jit_message(void) { return jit_message(); }
+uint64_t pcpd_jit_launch_count(void) { return jit_launch_count(); }
+
+int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_bytes)
+{
+    if (variant < 0 || variant > 3) return fail(PCPD_ERR_ARG, "jit_selftest: unknown variant %d", variant);
+    size_t n = 0;
+    if (jit_compile_only(variant, 7, 5, 4, 0, T_d, T_p, &n) != 0) return fail(PCPD_ERR_DEVICE, "%s", jit_message());
+    if (cubin_bytes) *cubin_bytes = n;
     return PCPD_OK;
 }
 

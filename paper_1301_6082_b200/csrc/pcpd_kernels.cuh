@@ -1,8 +1,10 @@
 // Kernel-side declarations shared by pcpd_kernels.cu (device code) and
 // pcpd_api.cu (host C ABI).  Product path only; nothing here is used by oracle/.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cstdint>
 #include <cuda_runtime.h>
+#endif
 
 #include "philox.cuh"
 
@@ -42,12 +44,29 @@ struct SweepParams {
     uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
 };
 
+#ifndef __CUDACC_RTC__
+// Threshold-specialised sweep kernel of one handle, compiled at run time (jit.cu).
+struct JitSlot {
+    int mode;      // 0 off, 1 auto (large problems only), 2 always (test hook)
+    int state;     // 0 not tried yet, 1 kernel ready, -1 unavailable (the built-in kernel is used)
+    void *kernel;  // CUfunction
+};
+
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.
-int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream);
+int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit);
 // warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);
-int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream);
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit);
+// jit.cu: compile (once per process, device and parameter set) sweep_warp_kernel<variant, wpb, nud, nup, pmode, 0, 1, Td, Tp>
+// with NVRTC and load it; NULL if NVRTC or the driver entry points are unavailable or the compilation fails
+// (message in jit_message()).  jit_launch returns a cudaError_t-like code (0 = launched).
+void *jit_sweep_kernel(int variant, int wpb, int nud, int nup, int pmode, uint32_t Td, uint32_t Tp, size_t max_smem);
+int jit_launch(void *kernel, const SweepParams &P, unsigned grid, unsigned block, size_t smem, cudaStream_t stream);
+const char *jit_message();
+uint64_t jit_launch_count();
+// compile only (no device needed): returns 0 and the cubin size; used by the CPU-side build check
+int jit_compile_only(int variant, int wpb, int nud, int nup, int pmode, uint32_t Td, uint32_t Tp, size_t *cubin_bytes);
 int configure_warp_kernels();
 int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,
                 const RoundKeys &rk, cudaStream_t stream);
@@ -63,5 +82,6 @@ size_t sweep_smem_bytes(uint32_t Ts, int Wb);
 
 // microbenchmarks (microbench.cu)
 int run_microbench(int kind, uint32_t iters, double *out_rate, cudaStream_t stream);
+#endif  // !__CUDACC_RTC__
 
 }  // namespace pcpd

@@ -2,7 +2,14 @@
 // the addressing of DESIGN.md section 3, C1-C2.  Device code of the product path;
 // shares nothing with oracle/.
 #pragma once
+#ifdef __CUDACC_RTC__
+// run-time compilation (jit.cu): no standard headers; NVRTC's own fixed-width built-in types
+typedef unsigned int uint32_t;
+typedef int int32_t;
+typedef unsigned long long uint64_t;
+#else
 #include <cstdint>
+#endif
 
 namespace pcpd {
 
@@ -25,6 +32,7 @@ struct RoundKeys {
     uint32_t k1[10];
 };
 
+#ifndef __CUDACC_RTC__
 inline RoundKeys make_round_keys(uint64_t seed)
 {
     RoundKeys rk;
@@ -37,6 +45,7 @@ inline RoundKeys make_round_keys(uint64_t seed)
     }
     return rk;
 }
+#endif
 
 struct U4 {
     uint32_t x0, x1, x2, x3;

@@ -1,461 +1,9 @@
-// sweep_warp_kernel - the production sweep kernel for sm_100a.
-//
-// Mapping: ONE WARP owns one (tile, word column) for a whole sweep; LANE b owns
-// domain b of that tile (n = T_s / D <= 32 domains).  The column's T_s words
-// live in shared memory from load to store, so the lattice crosses HBM exactly
-// once in each direction per sweep (0.25 B per replica-site update), with
-// coalesced 128-bit global accesses.  Because all domains of a tile column sit
-// in one warp, sub-steps need __syncwarp() only - no block barrier anywhere in
-// the sweep.
-//
-// Per attempt a lane issues, as one basic block, 1 + NU_D + NU_P independent Philox chains
-// (MISC block, the first NU_D DIFF blocks, the first NU_P ANNI blocks: none depends on the lattice
-// state) written round-major so that ptxas interleaves them; the planes are compared MSB-first
-// against T's bits on all 64 lanes in the signed-sum form (und chain on the ALU pipe, lt
-// accumulation as IMADs on the FMA pipe); the lazy tails then run as warp-uniform loops only while
-// some lane whose outcome can matter is undecided (DIFF: x or x+1 occupied; ANNI: reacting lanes).
-// Philox rounds 1-3 are strength-reduced: the products that depend only on (w, t) or only on the
-// slot are computed once per warp / once per attempt, leaving 16 IMAD.WIDE.U32 per block, not 20.
-//
-// Citations: update rule = Alg. 1 PAPER.md:45-70 in the bitwise form of Alg. 2
-// PAPER.md:126-151 (typos fixed per DESIGN.md readings G5/G6); schedule SD2 and
-// streams = DESIGN.md section 3 C1-C9.
-#include "pcpd_kernels.cuh"
+// sweep_warp.cu - host side of the production sweep kernel (device code: sweep_warp_device.cuh):
+// instantiations for the generic-threshold kernels built into libpcpd.so, launch configuration,
+// and the dispatch to the threshold-specialised kernels compiled at run time (jit.cu).
+#include "sweep_warp_device.cuh"
 
 namespace pcpd {
-
-namespace {
-
-__device__ __forceinline__ uint32_t hi32(uint64_t v) { return (uint32_t)(v >> 32); }
-__device__ __forceinline__ uint32_t lo32(uint64_t v) { return (uint32_t)v; }
-__device__ __forceinline__ uint64_t mulw(uint32_t a, uint32_t b) { return (uint64_t)a * b; }
-
-// Constants of one (sweep t, word w) pair: everything in rounds 1-3 that does
-// not depend on the slot or on c3.
-struct PhiloxWarp {
-    uint32_t B;     // lo(M1 w) ^ k0[1]
-    uint32_t C;     // hi(M0 c0') ^ k1[1],  c0' = hi(M1 w) ^ t ^ k0[0]
-    uint32_t Dc;    // lo(M0 c0') ^ k1[2]
-};
-
-__device__ __forceinline__ PhiloxWarp philox_warp_consts(uint32_t t, uint32_t w, const RoundKeys &rk)
-{
-    const uint64_t p1 = mulw(PHILOX_M1, w);
-    const uint32_t c0p = hi32(p1) ^ t ^ rk.k0[0];
-    const uint64_t p0p = mulw(PHILOX_M0, c0p);
-    PhiloxWarp pw;
-    pw.B = lo32(p1) ^ rk.k0[1];
-    pw.C = hi32(p0p) ^ rk.k1[1];
-    pw.Dc = lo32(p0p) ^ rk.k1[2];
-    return pw;
-}
-
-// Constants of one slot (attempt): 2 wide multiplies.
-struct PhiloxSlot {
-    uint32_t X;    // hi(M0 slot) ^ k1[0]           (c2' = X ^ c3)
-    uint32_t E;    // hi(M1 c2'') ^ k0[2],  c2'' = C ^ lo(M0 slot)
-    uint32_t c1;   // lo(M1 c2'')                    (c1 entering round 4)
-};
-
-__device__ __forceinline__ PhiloxSlot philox_slot_consts(uint32_t slot, const PhiloxWarp &pw, const RoundKeys &rk)
-{
-    const uint64_t p0 = mulw(PHILOX_M0, slot);
-    const uint32_t c2pp = pw.C ^ lo32(p0);
-    const uint64_t p1pp = mulw(PHILOX_M1, c2pp);
-    PhiloxSlot ps;
-    ps.X = hi32(p0) ^ rk.k1[0];
-    ps.E = hi32(p1pp) ^ rk.k0[2];
-    ps.c1 = lo32(p1pp);
-    return ps;
-}
-
-// Philox-4x32-10 block of counter (slot, t, w, c3): 16 IMAD.WIDE.U32 + 18 LOP3.
-__device__ __forceinline__ U4 philox_block(uint32_t c3, const PhiloxSlot &ps, const PhiloxWarp &pw,
-                                           const RoundKeys &rk)
-{
-    // round 1 -> only c2' depends on c3; round 2: one multiply; round 3: one multiply
-    const uint32_t c2p = ps.X ^ c3;
-    const uint64_t p1p = mulw(PHILOX_M1, c2p);
-    const uint32_t c0pp = hi32(p1p) ^ pw.B;
-    const uint64_t p0pp = mulw(PHILOX_M0, c0pp);
-    uint32_t c0 = ps.E ^ lo32(p1p);
-    uint32_t c1 = ps.c1;
-    uint32_t c2 = hi32(p0pp) ^ pw.Dc;
-    uint32_t c3r = lo32(p0pp);
-#pragma unroll
-    for (int r = 3; r < 10; ++r) {
-        const uint64_t p0 = mulw(PHILOX_M0, c0);
-        const uint64_t p1 = mulw(PHILOX_M1, c2);
-        const uint32_t n0 = hi32(p1) ^ c1 ^ rk.k0[r];
-        const uint32_t n2 = hi32(p0) ^ c3r ^ rk.k1[r];
-        c1 = lo32(p1);
-        c3r = lo32(p0);
-        c0 = n0;
-        c2 = n2;
-    }
-    return U4{c0, c1, c2, c3r};
-}
-
-// N blocks of one slot at once, written round-major / chain-minor so that the N
-// independent multiply chains are interleaved in the instruction stream (ptxas
-// keeps source order within its window; block-after-block code leaves the FMA
-// pipe waiting on one chain's latency).
-template <int N>
-__device__ __forceinline__ void philox_blocks(const uint32_t (&c3in)[N], const PhiloxSlot &ps, const PhiloxWarp &pw,
-                                              const RoundKeys &rk, U4 *out)
-{
-    uint32_t c0[N], c1[N], c2[N], c3[N];
-    uint64_t pa[N], pb[N];
-#pragma unroll
-    for (int i = 0; i < N; ++i) pa[i] = mulw(PHILOX_M1, ps.X ^ c3in[i]);
-#pragma unroll
-    for (int i = 0; i < N; ++i) pb[i] = mulw(PHILOX_M0, hi32(pa[i]) ^ pw.B);
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        c0[i] = ps.E ^ lo32(pa[i]);
-        c1[i] = ps.c1;
-        c2[i] = hi32(pb[i]) ^ pw.Dc;
-        c3[i] = lo32(pb[i]);
-    }
-#pragma unroll
-    for (int r = 3; r < 10; ++r) {
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            pa[i] = mulw(PHILOX_M0, c0[i]);
-            pb[i] = mulw(PHILOX_M1, c2[i]);
-        }
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            c0[i] = hi32(pb[i]) ^ c1[i] ^ rk.k0[r];
-            c2[i] = hi32(pa[i]) ^ c3[i] ^ rk.k1[r];
-            c1[i] = lo32(pb[i]);
-            c3[i] = lo32(pa[i]);
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < N; ++i) out[i] = U4{c0[i], c1[i], c2[i], c3[i]};
-}
-
-// Connected multispin lattice (C10): the successor of (site L-1, lane j) is
-// (site 0, lane j+1), so the words of the tile sites that lie past the ring wrap are rotated right by
-// one bit when the tile is loaded (bit j of the tile word = the strand that is in lane j before the
-// wrap) and rotated back when it is stored.  r is 0 or 1.
-__device__ __forceinline__ uint64_t rotr64(uint64_t v, uint32_t r) { return (v >> r) | (v << ((64u - r) & 63u)); }
-__device__ __forceinline__ uint64_t rotl64(uint64_t v, uint32_t r) { return (v << r) | (v >> ((64u - r) & 63u)); }
-
-// 64-lane mask state as two 32-bit halves.
-struct Mask2 {
-    uint32_t lo, hi;
-};
-__device__ __forceinline__ uint64_t m64(const Mask2 &m) { return (uint64_t)m.lo | ((uint64_t)m.hi << 32); }
-
-// MSB-first bit-sliced compare of two planes (p0 = plane 2m, p1 = plane 2m+1; block blk = planes
-// x0 | x1 << 32 and x2 | x3 << 32) against T's bits tb0, tb1 given as 32-lane masks (C3), in
-// signed-sum form.  und_k (lanes still equal to T before plane k) are nested
-// sets, and lt = OR_k (und_k - und_(k+1)) over the planes where T's bit is 1 = sum_k s_k * und_k with
-// s_k = tb_k - tb_(k-1) in {-1, 0, +1}: the lt accumulation becomes one 32-bit IMAD per plane and half
-// (FMA pipe, which has slack) and only the und chain (one LOP3 per plane and half) stays on the ALU
-// pipe, the binding one.  The caller closes the sum with -tb_last * und when it stops.
-__device__ __forceinline__ void cmp2h_sum(uint32_t &lt, uint32_t &und, uint32_t p0, uint32_t p1, uint32_t tb0,
-                                          uint32_t tb1, int32_t s0, int32_t s1)
-{
-    lt += und * (uint32_t)s0;
-    const uint32_t u1 = und & ~(p0 ^ tb0);
-    lt += u1 * (uint32_t)s1;
-    und = u1 & ~(p1 ^ tb1);
-}
-
-__device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &blk, uint32_t tb0, uint32_t tb1,
-                                              int32_t s0, int32_t s1)
-{
-    cmp2h_sum(lt.lo, und.lo, blk.x0, blk.x2, tb0, tb1, s0, s1);
-    cmp2h_sum(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1, s0, s1);
-}
-
-}  // namespace
-
-// NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
-// parameters so that the unconditional part has no branch at all): 5 and 4 for thresholds with that
-// many blocks (tuned on B200: a warp pays the maximum over its 32 lanes, so nearly every attempt
-// needs that many anyway), 1 for thresholds with few planes (d = 1/2 has one), 0 for T = 0 or 2^32.
-template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW>
-__global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
-{
-    extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
-
-    constexpr uint32_t Rr = VARIANT == 3 ? 1u : 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
-    const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
-
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
-    const uint32_t ntiles = L / Ts;
-    const uint32_t task = blockIdx.x * WPB + warp;
-    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel
-
-    // C5 step 1: shifts from the SHIFT stream; lane j holds sigma_{k0+j} of the current group of 32 sub-steps.
-    uint32_t sig_reg, Sigma;
-    {
-        const U4 blk = philox4x32_10(lane, t, 0u, STREAM_SHIFT, P.rk);
-        sig_reg = __umulhi(blk.x0, D);
-        Sigma = __shfl_sync(0xffffffffu, __umulhi(blk.x1, Ts), 0);
-    }
-    const uint32_t tau = task % ntiles, wl = task / ntiles;
-    const uint32_t w = P.word_offset + wl;  // global word index (RNG key)
-
-    // ---- C5 step 2: tile tau covers global sites (Sigma + tau*Ts + y) mod L ----
-    const uint32_t start = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts) % L);
-    uint64_t *g = P.lat + (size_t)wl * L;             // column wl, contiguous in the site index
-    const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
-    uint64_t *buf = smem + (size_t)warp * stride;
-    const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
-    const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
-    const uint32_t odd = vec ? (start & 1u) : 0u;
-    uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
-    if (vec) {
-        const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
-        const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
-        ulonglong2 *b2 = reinterpret_cast<ulonglong2 *>(buf);
-#pragma unroll 8
-        for (uint32_t pi = lane; pi < npairs; pi += 32) {
-            uint32_t i = s0 + 2 * pi;
-            if (i >= L) i -= L;
-            b2[pi] = g2[i >> 1];
-        }
-        if (conn && s0 + 2 * npairs > L) {
-            // connected lattice: rotate the words past the ring wrap in place (L and s0 are even, so
-            // both words of a pair lie on the same side of the wrap)
-            __syncwarp();
-            for (uint32_t k2 = (L - s0) + lane; k2 < 2 * npairs; k2 += 32) buf[k2] = rotr64(buf[k2], 1u);
-        }
-    } else {
-        for (uint32_t y = lane; y < Ts; y += 32) {
-            uint32_t i = start + y;
-            if (i >= L) i -= L;
-            tile[y] = g[i];
-        }
-        if (conn && start + Ts > L) {
-            __syncwarp();
-            for (uint32_t y = (L - start) + lane; y < Ts; y += 32) tile[y] = rotr64(tile[y], 1u);
-        }
-    }
-    __syncwarp();
-
-    const PhiloxWarp pw = philox_warp_consts(t, w, P.rk);
-    const bool act = lane < n;
-    const uint32_t b = act ? lane : 0u;
-    const uint32_t slot0 = (tau * n + b) * D;
-    uint32_t nblkD = (P.thd.nplanes + 1u) >> 1, nblkP = (P.thp.nplanes + 1u) >> 1;
-    uint32_t Td = P.thd.T32, Tp = P.thp.T32;
-    bool allD = P.thd.all != 0, allP = P.thp.all != 0;
-    // Per-word thresholds (C11): the bit masks and signed-sum coefficients of the unconditional planes live in
-    // registers for the whole task instead of the constant bank.  Planes past a word's last significant one have
-    // T bit 0, which closes the signed sum at the right plane by itself.
-    uint32_t tdm_r[2 * NU_D + 1], tpm_r[2 * NU_P + 1];
-    int32_t sd_r[2 * NU_D + 1], sp_r[2 * NU_P + 1];
-    if constexpr (PW) {
-        const uint4 th = reinterpret_cast<const uint4 *>(P.thr_dev)[wl];
-        Td = th.x; Tp = th.y; allD = (th.z & 1u) != 0; allP = (th.z & 2u) != 0;
-        nblkD = Td ? (32u - (uint32_t)(__ffs((int)Td) - 1) + 1u) >> 1 : 0u;
-        nblkP = Tp ? (32u - (uint32_t)(__ffs((int)Tp) - 1) + 1u) >> 1 : 0u;
-#pragma unroll
-        for (int kk = 0; kk < 2 * NU_D; ++kk) {
-            const uint32_t bit = (Td >> (31 - kk)) & 1u, prev = kk ? (Td >> (32 - kk)) & 1u : 0u;
-            tdm_r[kk] = 0u - bit;
-            sd_r[kk] = (int32_t)bit - (int32_t)prev;
-        }
-#pragma unroll
-        for (int kk = 0; kk < 2 * NU_P; ++kk) {
-            const uint32_t bit = (Tp >> (31 - kk)) & 1u, prev = kk ? (Tp >> (32 - kk)) & 1u : 0u;
-            tpm_r[kk] = 0u - bit;
-            sp_r[kk] = (int32_t)bit - (int32_t)prev;
-        }
-    }
-
-    for (uint32_t k = 0; k < S; ++k) {
-        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, P.rk).x0, D);
-        const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
-        // C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
-        // domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
-        const bool seam = (b == n - 1) && (sigma > 0);
-        const int32_t c = (int32_t)D - (int32_t)sigma;
-        int32_t lo = 0, rem = 0;
-        if (seam) {
-            lo = max(1, c - (int32_t)Rr);
-            const int32_t hi = min((int32_t)D - 1 - (int32_t)Rr, c);
-            rem = max(0, hi - lo + 1);
-        }
-        const uint32_t n_allow = D - 1 - Rr - (uint32_t)rem;
-        const uint32_t dbase = sigma + b * D;  // tile-local index of domain-local 0 (before wrap)
-
-        for (uint32_t a = 0; a < A; ++a) {
-            // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
-            // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
-            // back to back so that the FMA pipe always has several wide multiplies in flight.
-            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, P.rk);
-            uint32_t c3s[1 + NU_D + NU_P];
-            U4 blks[1 + NU_D + NU_P];
-            c3s[0] = STREAM_MISC;
-#pragma unroll
-            for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
-#pragma unroll
-            for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
-            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, P.rk, blks);
-            const U4 misc = blks[0];
-            const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
-
-            // C4: MISC block: Fm = ~lo (1 -> fission low, Alg. 1: r3 < 1/2), x2 -> position.
-            int32_t x = 1 + (int32_t)__umulhi(misc.x2, n_allow);
-            if (rem > 0 && x >= lo) x += rem;
-            uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
-            if (y0 >= Ts) y0 -= Ts;
-            const uint64_t Fm = ~lo64(misc);
-            uint64_t *q = tile + y0;
-            uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0, sg = 0;
-            if (act) {
-                sa = q[0]; sb = q[1]; sc = q[2];
-                if constexpr (VARIANT != 3) se = q[3];
-                if constexpr (VARIANT == 1 || VARIANT == 2) sf = q[4];
-                if constexpr (VARIANT == 2) sg = q[5];
-            }
-
-            // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
-            // dependence on the state), the lazy tails only on the lanes whose outcome can matter:
-            // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
-            Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-#pragma unroll
-            for (int m = 0; m < NU_D; ++m)
-                cmp_block_sum(dlt, dund, dblk[m], PW ? tdm_r[2 * m] : P.tdm[2 * m], PW ? tdm_r[2 * m + 1] : P.tdm[2 * m + 1],
-                              PW ? sd_r[2 * m] : P.sd[2 * m], PW ? sd_r[2 * m + 1] : P.sd[2 * m + 1]);
-            if constexpr (PMODE == 0) {
-#pragma unroll
-                for (int m = 0; m < NU_P; ++m)
-                    cmp_block_sum(plt, pund, pblk[m], PW ? tpm_r[2 * m] : P.tpm[2 * m],
-                                  PW ? tpm_r[2 * m + 1] : P.tpm[2 * m + 1], PW ? sp_r[2 * m] : P.sp[2 * m],
-                                  PW ? sp_r[2 * m + 1] : P.sp[2 * m + 1]);
-            }
-            {
-                const uint64_t rel = sb | sc;
-                dund.lo &= (uint32_t)rel;
-                dund.hi &= (uint32_t)(rel >> 32);
-                uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top (0 past the last plane)
-                uint32_t m = NU_D;
-                int32_t prev = NU_D > 0 ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;  // T's bit of the last plane done (PW)
-                for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
-                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, P.rk);
-                    int32_t s0, s1;
-                    if constexpr (PW) {
-                        const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
-                        s0 = b0 - prev; s1 = b1 - b0; prev = b1;
-                    } else {
-                        s0 = P.sd[2 * m]; s1 = P.sd[2 * m + 1];
-                    }
-                    cmp_block_sum(dlt, dund, blk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31), s0, s1);
-                    Tsh <<= 2;
-                }
-                // close the sum: lanes still equal to T after the last plane looked at are not < T
-                const uint32_t cl = PW ? (uint32_t)(-prev) : (uint32_t)P.cld[m];
-                dlt.lo += dund.lo * cl;
-                dlt.hi += dund.hi * cl;
-            }
-            const uint64_t Dm = allD ? ~0ull : m64(dlt);
-            uint64_t react = sb & ~Dm;  // particle cluster (1, 2, 3 or 4 sites from x) present and no diffusion
-            if constexpr (VARIANT != 3) react &= sc;
-            if constexpr (VARIANT == 1 || VARIANT == 2) react &= se;
-            if constexpr (VARIANT == 2) react &= sf;
-            if constexpr (PMODE == 0) {
-                pund.lo &= (uint32_t)react;
-                pund.hi &= (uint32_t)(react >> 32);
-                uint32_t Tsh = Tp << (2 * NU_P);
-                uint32_t m = NU_P;
-                int32_t prev = NU_P > 0 ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
-                for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
-                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, P.rk);
-                    int32_t s0, s1;
-                    if constexpr (PW) {
-                        const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
-                        s0 = b0 - prev; s1 = b1 - b0; prev = b1;
-                    } else {
-                        s0 = P.sp[2 * m]; s1 = P.sp[2 * m + 1];
-                    }
-                    cmp_block_sum(plt, pund, bk, (uint32_t)((int32_t)Tsh >> 31), (uint32_t)((int32_t)(Tsh << 1) >> 31), s0, s1);
-                    Tsh <<= 2;
-                }
-                const uint32_t cl = PW ? (uint32_t)(-prev) : (uint32_t)P.clp[m];
-                plt.lo += pund.lo * cl;
-                plt.hi += pund.hi * cl;
-            } else {
-                // The paper's own annihilation mask (Alg. 2 lines 12-13):
-                // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
-                // word-wide draw that is 1 w.p. 4p (x3 of the MISC block against floor(4p * 2^32)).
-                const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-                plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
-                plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
-            }
-            const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);
-
-            // C6 / Alg. 2, branch-free over the 64 replicas.
-            uint64_t nb = (Dm & sc) | (~Dm & sb);
-            uint64_t nc = (Dm & sb) | (~Dm & sc);
-            const uint64_t ann = react & Pm;
-            const uint64_t fis = react & ~Pm;
-            nb &= ~ann;
-            if constexpr (VARIANT != 3) nc &= ~ann;
-            sa |= fis & Fm;
-            if (act) {
-                if constexpr (VARIANT == 3) {        // CPD: single particle at x; fission high -> x+1 (react lanes have Dm = 0)
-                    nc |= fis & ~Fm;
-                } else if constexpr (VARIANT == 0) { // PCPD: pair at x, x+1; fission high -> x+2
-                    se |= fis & ~Fm;
-                } else if constexpr (VARIANT == 1) { // TCPD: triple x..x+2; high -> x+3
-                    se &= ~ann;
-                    sf |= fis & ~Fm;
-                    q[4] = sf;
-                } else {                             // QCPD: quadruplet x..x+3; high -> x+4
-                    se &= ~ann;
-                    sf &= ~ann;
-                    sg |= fis & ~Fm;
-                    q[4] = sf;
-                    q[5] = sg;
-                }
-                q[0] = sa; q[1] = nb; q[2] = nc;
-                if constexpr (VARIANT != 3) q[3] = se;
-            }
-        }
-        __syncwarp();
-    }
-
-    // ---- store the tile ----
-    if (conn) {  // connected lattice: rotate the words past the ring wrap back (see the load)
-        const uint32_t first = vec ? (start - odd) : start, nw = vec ? 2 * (Ts / 2 + odd) : Ts;
-        uint64_t *base = vec ? buf : tile;
-        if (first + nw > L) {
-            for (uint32_t k2 = (L - first) + lane; k2 < nw; k2 += 32) base[k2] = rotl64(base[k2], 1u);
-            __syncwarp();
-        }
-    }
-    if (vec) {
-        const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
-        ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
-        const ulonglong2 *b2 = reinterpret_cast<const ulonglong2 *>(buf);
-#pragma unroll 8
-        for (uint32_t pi = lane; pi < npairs; pi += 32) {
-            uint32_t i = s0 + 2 * pi;
-            if (i >= L) i -= L;
-            if (odd && (pi == 0 || pi == npairs - 1)) {
-                // edge pairs of an odd-aligned tile hold one foreign word each
-                if (pi == 0) g[i + 1] = buf[1];
-                else g[i] = buf[2 * pi];
-            } else {
-                g2[i >> 1] = b2[pi];
-            }
-        }
-    } else {
-        for (uint32_t y = lane; y < Ts; y += 32) {
-            uint32_t i = start + y;
-            if (i >= L) i -= L;
-            g[i] = tile[y];
-        }
-    }
-}
 
 // ---------------------------------------------------------------------------
 static size_t warp_smem_bytes(uint32_t Ts, int wpb) { return (size_t)wpb * ((Ts + 3u) & ~1u) * 8; }
@@ -526,11 +74,28 @@ static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams
     return wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream) : warp_op_d<1, 1>(nud, nup, P, stream);
 }
 
-int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream)
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit)
 {
     if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
-    return warp_op_any(variant, wpb, nu_d_of((P.thd.nplanes + 1) >> 1), nup, &P, stream);
+    const int nud = nu_d_of((P.thd.nplanes + 1) >> 1);
+    // Threshold-specialised kernel (jit.cu): large problems (wpb == 7), or every size with PCPD_JIT=force.  Not
+    // for T = 2^32 (d = 1 or p = 1; the template constants hold 32 bits).  If it cannot be had, the built-in
+    // kernel below computes the same thing.
+    if (jit && jit->mode && jit->state >= 0 && (jit->mode == 2 || wpb == 7) && !P.thd.all && !P.thp.all) {
+        if (jit->state == 0) {
+            jit->kernel = jit_sweep_kernel(variant, wpb, nud, P.pmask_paper ? 1 : nup, P.pmask_paper ? 1 : 0, P.thd.T32,
+                                           P.thp.T32, wpb >= 4 ? 116 * 1024 : 226 * 1024);
+            jit->state = jit->kernel ? 1 : -1;
+        }
+        if (jit->state == 1) {
+            const uint32_t ntasks = (P.L / P.Ts) * P.W;
+            if (jit_launch(jit->kernel, P, (ntasks + wpb - 1) / wpb, wpb * 32, warp_smem_bytes(P.Ts, wpb), stream) == 0)
+                return 1;
+            jit->state = -1;
+        }
+    }
+    return warp_op_any(variant, wpb, nud, nup, &P, stream);
 }
 
 int configure_warp_kernels()

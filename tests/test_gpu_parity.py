@@ -55,7 +55,7 @@ def oracle_columns(cfg_kw, words, init, n_sweeps_list, words_in=None):
     return out
 
 
-def gpu_check(pk, kw, sch, init, times, words=None, words_in=None):
+def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=False):
     W = kw["n_replicas"] // 64
     words = list(range(W)) if words is None else words
     okw = dict(kw)
@@ -80,6 +80,8 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None):
         if bits is not None:
             assert np.array_equal(bits.sum(axis=0).ravel().astype(np.uint32), cnt)
     assert g.sweep == times[-1]
+    if expect_jit:  # the sweeps ran the threshold-specialised (run-time compiled) kernel, not the built-in one
+        assert g.jit_state() == 1, pk.jit_message()
     g.close()
 
 
@@ -133,6 +135,40 @@ def test_small_cases_bit_exact_every_sweep(pk, case):
     variant, L, R, d, p, Ts, D, A, init = case
     kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
     gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)))
+
+
+# cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
+JIT_CASES = [0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12, 14, 16, 17, 18, 19, 20, 22, 23, 25, 26, 27, 29]
+
+
+@pytest.mark.parametrize("idx", JIT_CASES, ids=[f"case{i}" for i in JIT_CASES])
+def test_threshold_specialised_kernel_bit_exact_every_sweep(pk, idx, monkeypatch):
+    """The run-time compiled sweep kernel (T_d, T_p as template constants; csrc/jit.cu), forced on at small
+    sizes with PCPD_JIT=force: same bar as the built-in kernel - every word and count after every sweep."""
+    monkeypatch.setenv("PCPD_JIT", "force")
+    variant, L, R, d, p, Ts, D, A, init = SMALL[idx]
+    kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
+    n0 = pk.jit_launch_count()
+    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)), expect_jit=True)
+    assert pk.jit_launch_count() - n0 == 6
+
+
+def test_specialised_and_builtin_kernels_agree_at_full_size(pk, monkeypatch):
+    """cfg4 and cfg5 whole lattices: the run-time specialised kernel (default at this size) against the
+    built-in generic-threshold kernel (PCPD_JIT=0)."""
+    for name in ("cfg4", "cfg5"):
+        c = wl.BY_NAME[name]
+        res = []
+        for mode in ("1", "0"):
+            monkeypatch.setenv("PCPD_JIT", mode)
+            g = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
+            g.init(c.init)
+            g.run(3)
+            assert g.jit_state() == (1 if mode == "1" else 0), pk.jit_message()
+            res.append((g.get_lattice(), g.density()))
+            g.close()
+        monkeypatch.delenv("PCPD_JIT")
+        assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
 
 
 def test_hand_built_lattice_and_seed_high_bits(pk):
@@ -220,7 +256,9 @@ def test_full_size_configs_sampled_columns(pk, name, words, horizon):
     c = wl.BY_NAME[name]
     kw = dict(L=c.L, n_replicas=c.n_replicas, d=c.d, p=c.p, seed=c.seed, variant=c.variant)
     times = [t for t in (1, 2, 4) if t <= horizon]
-    gpu_check(pk, kw, {}, c.init, times, words=words)
+    n0 = pk.jit_launch_count()
+    gpu_check(pk, kw, {}, c.init, times, words=words, expect_jit=True)
+    assert pk.jit_launch_count() - n0 == times[-1]
 
 
 def test_philox_block_via_init_stream(pk):

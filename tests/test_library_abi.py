@@ -54,6 +54,19 @@ def test_argument_errors_without_device(lib):
     lib.pcpd_destroy(None)  # NULL-safe
 
 
+@pytest.mark.parametrize("variant,Td,Tp", [(0, 0xCCCCCCCC, 0x1EB851EB), (1, 0x80000000, 0x0CCCCCCC), (2, 1, 0xFFFFFFFF),
+                                           (3, 0, 0x4CCCCCCC)])
+def test_run_time_specialisation_compiles_for_sm_100a(lib, variant, Td, Tp):
+    """csrc/jit.cu: the device source embedded in the library compiles with NVRTC for sm_100a with the
+    thresholds as template constants (needs libnvrtc, no device)."""
+    n = C.c_uint64(0)
+    rc = lib.pcpd_jit_selftest(variant, Td, Tp, C.byref(n))
+    if rc != 0 and b"libnvrtc not found" in lib.pcpd_last_error():
+        pytest.skip("libnvrtc is not installed here")
+    assert rc == 0, lib.pcpd_last_error()
+    assert n.value > 10_000  # a cubin, not an empty image
+
+
 def test_no_cpu_fallback_without_gpu():
     import torch
 
