@@ -165,12 +165,14 @@ PCPD_API const char *pcpd_last_error(void);              /* thread-local, librar
  * d and p are constants for the life of a handle, and the kernel's compare of the random planes with
  * the bits of T_d, T_p (C3) is cheaper when those bits are compile-time constants.  For large problems
  * (at least 148 x 14 tile columns) the first pcpd_run of a handle therefore compiles the SAME device
- * source with T_d, T_p as template constants (NVRTC, sm_100a; about a second, once per process, device
- * and parameter set) and runs that kernel from then on.  Results are identical bit for bit.  If
+ * source with T_d, T_p - and the schedule constants T_s, D, A and L - as template constants (NVRTC,
+ * sm_100a; about a second, once per process, device and parameter set) and runs that kernel from then on.  Results are identical bit for bit.  If
  * libnvrtc cannot be loaded or the compilation fails, the handle keeps the built-in generic-threshold
  * CUDA kernel (this is not a CPU fallback) and pcpd_jit_message() says why.  Environment, read by
  * pcpd_create*: PCPD_JIT=0 never specialise; PCPD_JIT=force specialise at every problem size (test
- * hook); PCPD_NVRTC_PATH = full path of libnvrtc.so.12 if it is not on the loader path.  Not used with
+ * hook); PCPD_NVRTC_PATH = full path of libnvrtc.so.12 if it is not on the loader path; tuning /
+ * inspection hooks PCPD_JIT_NUD, PCPD_JIT_NUP (prefix lengths), PCPD_JIT_OPTS (extra NVRTC options),
+ * PCPD_JIT_DUMP (file to keep the cubin in, for cuobjdump -sass).  Not used with
  * per-word-column probabilities (pcpd_create_scan), nor when d = 1 or p = 1.
  * pcpd_jit_state: 1 the handle's sweeps run the specialised kernel; 0 not tried (no sweep yet) or not
  * applicable; -1 tried and unavailable.  pcpd_jit_launch_count: specialised-kernel launches of this

@@ -455,7 +455,12 @@ int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_b
 {
     if (variant < 0 || variant > 3) return fail(PCPD_ERR_ARG, "jit_selftest: unknown variant %d", variant);
     size_t n = 0;
-    if (jit_compile_only(variant, 7, 5, 4, 0, T_d, T_p, &n) != 0) return fail(PCPD_ERR_DEVICE, "%s", jit_message());
+    JitSpec js;
+    js.variant = variant; js.wpb = 7; js.pmode = 0;
+    js.nud = T_d ? (int)((32 - __builtin_ctz(T_d) + 1) / 2 < 6 ? (32 - __builtin_ctz(T_d) + 1) / 2 : 6) : 0;
+    js.nup = T_p ? (int)((32 - __builtin_ctz(T_p) + 1) / 2 < 4 ? (32 - __builtin_ctz(T_p) + 1) / 2 : 4) : 0;
+    js.Td = T_d; js.Tp = T_p; js.Ts = PCPD_DEFAULT_TS; js.D = PCPD_DEFAULT_D; js.A = PCPD_DEFAULT_A; js.L = 1u << 20;
+    if (jit_compile_only(js, &n) != 0) return fail(PCPD_ERR_DEVICE, "%s", jit_message());
     if (cubin_bytes) *cubin_bytes = n;
     return PCPD_OK;
 }

@@ -58,15 +58,19 @@ int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cud
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit);
-// jit.cu: compile (once per process, device and parameter set) sweep_warp_kernel<variant, wpb, nud, nup, pmode, 0, 1, Td, Tp>
-// with NVRTC and load it; NULL if NVRTC or the driver entry points are unavailable or the compilation fails
+// jit.cu: compile (once per process, device and parameter set)
+// sweep_warp_kernel<variant, wpb, nud, nup, pmode, 0, 1, Td, Tp, Ts, D, A, L> with NVRTC and load it; NULL if NVRTC or the driver entry points are unavailable or the compilation fails
 // (message in jit_message()).  jit_launch returns a cudaError_t-like code (0 = launched).
-void *jit_sweep_kernel(int variant, int wpb, int nud, int nup, int pmode, uint32_t Td, uint32_t Tp, size_t max_smem);
+struct JitSpec {
+    int variant, wpb, nud, nup, pmode;
+    uint32_t Td, Tp, Ts, D, A, L;
+};
+void *jit_sweep_kernel(const JitSpec &js, size_t max_smem);
 int jit_launch(void *kernel, const SweepParams &P, unsigned grid, unsigned block, size_t smem, cudaStream_t stream);
 const char *jit_message();
 uint64_t jit_launch_count();
 // compile only (no device needed): returns 0 and the cubin size; used by the CPU-side build check
-int jit_compile_only(int variant, int wpb, int nud, int nup, int pmode, uint32_t Td, uint32_t Tp, size_t *cubin_bytes);
+int jit_compile_only(const JitSpec &js, size_t *cubin_bytes);
 int configure_warp_kernels();
 int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,
                 const RoundKeys &rk, cudaStream_t stream);

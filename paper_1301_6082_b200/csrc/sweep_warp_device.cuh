@@ -216,14 +216,20 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
 // needs that many anyway), 1 for thresholds with few planes (d = 1/2 has one), 0 for T = 0 or 2^32.
 //
 // SPEC = 1 (kernels compiled at run time by jit.cu): the thresholds are the template constants STD, STP
-// (low 32 bits of T_d, T_p; neither threshold is 2^32) instead of P.thd / P.thp and the host tables.
-template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW, int SPEC = 0, uint32_t STD = 0u, uint32_t STP = 0u>
+// (low 32 bits of T_d, T_p; neither threshold is 2^32) instead of P.thd / P.thp and the host tables, and
+// the schedule constants T_s, D, A and the ring length L are the template constants CTS, CD, CA, CL.
+template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW, int SPEC = 0, uint32_t STD = 0u, uint32_t STP = 0u,
+          uint32_t CTS = 0u, uint32_t CD = 0u, uint32_t CA = 0u, uint32_t CL = 0u>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
 
     constexpr uint32_t Rr = VARIANT == 3 ? 1u : 2u + VARIANT;  // right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
-    const uint32_t Ts = P.Ts, D = P.D, A = P.A, S = P.S, n = P.n, L = P.L, t = P.t;
+    // SPEC kernels also have the schedule constants and the ring length as template constants (address
+    // arithmetic, seam bookkeeping and the mulhi by n_allow then work on immediates).
+    const uint32_t Ts = SPEC ? CTS : P.Ts, D = SPEC ? CD : P.D, A = SPEC ? CA : P.A, L = SPEC ? CL : P.L;
+    const uint32_t S = SPEC ? CD / (CA ? CA : 1u) : P.S, n = SPEC ? CTS / (CD ? CD : 1u) : P.n, t = P.t;
+    const RoundKeys &rk = P.rk;  // (baking the seed in as well was measured slower: 32-bit immediates in the xor chain)
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     const uint32_t ntiles = L / Ts;
@@ -233,7 +239,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     // C5 step 1: shifts from the SHIFT stream; lane j holds sigma_{k0+j} of the current group of 32 sub-steps.
     uint32_t sig_reg, Sigma;
     {
-        const U4 blk = philox4x32_10(lane, t, 0u, STREAM_SHIFT, P.rk);
+        const U4 blk = philox4x32_10(lane, t, 0u, STREAM_SHIFT, rk);
         sig_reg = __umulhi(blk.x0, D);
         Sigma = __shfl_sync(0xffffffffu, __umulhi(blk.x1, Ts), 0);
     }
@@ -278,7 +284,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     }
     __syncwarp();
 
-    const PhiloxWarp pw = philox_warp_consts(t, w, P.rk);
+    const PhiloxWarp pw = philox_warp_consts(t, w, rk);
     const bool act = lane < n;
     const uint32_t b = act ? lane : 0u;
     const uint32_t slot0 = (tau * n + b) * D;
@@ -313,8 +319,9 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 
+#pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
-        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, P.rk).x0, D);
+        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
         const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
         // C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
         // domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
@@ -329,11 +336,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         const uint32_t n_allow = D - 1 - Rr - (uint32_t)rem;
         const uint32_t dbase = sigma + b * D;  // tile-local index of domain-local 0 (before wrap)
 
+#pragma unroll 1
         for (uint32_t a = 0; a < A; ++a) {
             // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
             // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
             // back to back so that the FMA pipe always has several wide multiplies in flight.
-            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, P.rk);
+            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
             uint32_t c3s[1 + NU_D + NU_P];
             U4 blks[1 + NU_D + NU_P];
             c3s[0] = STREAM_MISC;
@@ -341,7 +349,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
 #pragma unroll
             for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
-            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, P.rk, blks);
+            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, rk, blks);
             const U4 misc = blks[0];
             const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
 
@@ -389,7 +397,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
-                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, P.rk);
+                    const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
                         const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
@@ -417,7 +425,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t m = NU_P;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
-                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, P.rk);
+                    const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
                         const int32_t b0 = (int32_t)(Tsh >> 31), b1 = (int32_t)((Tsh >> 30) & 1u);
