@@ -57,28 +57,36 @@ def nplanes_of(q: float) -> int:
     return 32 - ((T & -T).bit_length() - 1)
 
 
-# Per-block and fixed thread-instruction counts of the sweep kernel's own SASS (sweep_warp.cu, nvcc 12.9):
-# one strength-reduced Philox-4x32-10 block = 16 IMAD.WIDE.U32 + 18 LOP3; MSB-first compare of its two planes
-# = 8 instructions (per plane and 32-lane half one LOP3 for the und chain + one 32-bit IMAD for the signed-sum lt);
-# per attempt: 2 IMAD.WIDE (slot constants) + 1 IMAD.HI (position) and ~40 logic/address ops (rule 22,
-# position/seam/address 12, tail masks 6; TCPD +6).
-WIDE_PER_BLOCK, ALU_PER_BLOCK = 16.0, 18.0 + 8.0
+# Per-block and fixed thread-instruction counts of the sweep kernel's own SASS (sweep_warp_device.cuh, nvcc 12.9):
+# one strength-reduced Philox-4x32-10 block = 16 IMAD.WIDE.U32 + 18 LOP3; MSB-first compare of its two planes with T
+# = 8 instructions (per plane and 32-lane half one LOP3 for the und chain + one 32-bit IMAD for the signed-sum lt;
+# the run-time specialised kernel needs 4 in its prefix - the yardstick keeps the generic 8).  The MISC block has no
+# threshold compare (Fm = ~lo folds into the rule's truth tables); the ANNI block of the paper's annihilation mask
+# takes 4 LOP3 (two planes ANDed and gated, per half) instead of a compare.  Per attempt: 2 IMAD.WIDE (slot
+# constants) + 1 IMAD.HI (position) and ~40 logic/address ops (rule 22, position/seam/address 12, tail masks 6; TCPD +6).
+WIDE_PER_BLOCK, LOP_PER_BLOCK, CMP_PER_BLOCK, PMASK_PER_BLOCK = 16.0, 18.0, 8.0, 4.0
 WIDE_FIXED = 3.0
 
 
 def algorithmic_instr_per_attempt_word(cfg: wl.Config) -> dict:
     alu_fixed = 40.0 if (cfg.variant & 0xff) == wl.PCPD else 46.0
     npd, npp = nplanes_of(cfg.d), nplanes_of(cfg.p)
-    if cfg.variant & wl.PMASK_PAPER:   # the paper's annihilation mask: ANNI block 0 only (two planes ANDed + gate)
-        lazy_blocks = 1.0 + blocks_needed_generic(npd) + 1.0
-        eager_blocks = 1.0 + (npd + 1) // 2 + 1.0
-    else:
-        lazy_blocks = 1.0 + blocks_needed_generic(npd) + blocks_needed_generic(npp)   # + the MISC block
-        eager_blocks = 1.0 + (npd + 1) // 2 + (npp + 1) // 2
-    per_block = WIDE_PER_BLOCK + ALU_PER_BLOCK
+    raw = WIDE_PER_BLOCK + LOP_PER_BLOCK        # a block whose planes are used as they are (MISC)
+    cmp_blk = raw + CMP_PER_BLOCK               # a block whose two planes are compared with T
     fixed = WIDE_FIXED + alu_fixed
-    return dict(lazy=fixed + per_block * lazy_blocks, eager=fixed + per_block * eager_blocks,
-                lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=fixed, per_block=per_block)
+    if cfg.variant & wl.PMASK_PAPER:   # the paper's annihilation mask: ANNI block 0 only (two planes ANDed + gate)
+        lazy_d, eager_d = blocks_needed_generic(npd), (npd + 1) // 2
+        lazy = fixed + raw + cmp_blk * lazy_d + (raw + PMASK_PER_BLOCK)
+        eager = fixed + raw + cmp_blk * eager_d + (raw + PMASK_PER_BLOCK)
+        lazy_blocks, eager_blocks = 2.0 + lazy_d, 2.0 + eager_d
+    else:
+        lazy_dp = blocks_needed_generic(npd) + blocks_needed_generic(npp)
+        eager_dp = (npd + 1) // 2 + (npp + 1) // 2
+        lazy = fixed + raw + cmp_blk * lazy_dp
+        eager = fixed + raw + cmp_blk * eager_dp
+        lazy_blocks, eager_blocks = 1.0 + lazy_dp, 1.0 + eager_dp   # + the MISC block
+    return dict(lazy=lazy, eager=eager, lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=fixed,
+                per_block=cmp_blk)
 
 
 def variant_name(v: int) -> str:
