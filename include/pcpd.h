@@ -184,6 +184,16 @@ PCPD_API const char *pcpd_jit_message(void);
 PCPD_API uint64_t pcpd_jit_launch_count(void);
 PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_bytes);
 
+/* ---- small problems: two kernels per sweep -----------
+ * With fewer tile columns ((L / T_s) * W) than the GPU has warp slots to fill, one warp per tile column leaves
+ * the machine idle and each sweep is the latency of one warp's chain of D attempts.  Such handles (at most 592
+ * tile columns by default) run each sweep as two launches: mask_kernel computes the state-independent part of
+ * ALL attempts of the sweep in parallel (MISC block, compared prefix planes of DIFF and ANNI), then the update
+ * kernel reads them and applies the attempts in order.  Same results bit for bit.  Environment, read by
+ * pcpd_create*: PCPD_SPLIT=0 never; PCPD_SPLIT=force whenever the mask buffer stays below 1 GiB (test hook).
+ * pcpd_split_launch_count: kernels this handle has launched on that path (2 per sweep; 0 = fused kernel). */
+PCPD_API uint64_t pcpd_split_launch_count(const pcpd_t *h);
+
 /* Number of kernels this library has launched so far in this process. */
 PCPD_API uint64_t pcpd_launch_count(void);
 

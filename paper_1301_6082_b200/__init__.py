@@ -34,7 +34,7 @@ EXPORTS = (
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
-    "pcpd_jit_selftest",
+    "pcpd_jit_selftest", "pcpd_split_launch_count",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -118,6 +118,8 @@ def load_library() -> C.CDLL:
     L.pcpd_jit_launch_count.restype = C.c_uint64
     L.pcpd_jit_selftest.argtypes = [C.c_int, C.c_uint32, C.c_uint32, u64p]
     L.pcpd_jit_selftest.restype = C.c_int
+    L.pcpd_split_launch_count.argtypes = [C.c_void_p]
+    L.pcpd_split_launch_count.restype = C.c_uint64
     _lib = L
     return L
 
@@ -280,6 +282,10 @@ class Pcpd:
     @sweep.setter
     def sweep(self, t):
         _check(self._lib, self._lib.pcpd_set_sweep(self._h, t))
+
+    def split_launch_count(self) -> int:
+        """Kernels launched on the two-kernel small-problem path (2 per sweep; 0: fused kernel)."""
+        return int(self._lib.pcpd_split_launch_count(self._h))
 
     def jit_state(self) -> int:
         """1: sweeps run the threshold-specialised kernel; 0: not tried / not applicable; -1: unavailable."""

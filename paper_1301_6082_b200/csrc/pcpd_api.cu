@@ -14,6 +14,11 @@
 
 using namespace pcpd;
 
+// SPLIT path (small problems): largest number of tile columns it is used for by default (tuned on B200)
+#ifndef PCPD_SPLIT_MAX_TASKS
+#define PCPD_SPLIT_MAX_TASKS 592u
+#endif
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -85,6 +90,7 @@ struct pcpd_s {
     cudaStream_t stream;
     SweepParams P;
     JitSlot jit;       // threshold-specialised sweep kernel (jit.cu); mode from env PCPD_JIT at create
+    SplitSlot split;   // small problems: mask buffer of the two-kernel sweep (sweep_warp.cu); env PCPD_SPLIT
 };
 
 extern "C" {
@@ -210,6 +216,8 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         h->jit.state = 0;
         h->jit.kernel = nullptr;
     }
+    h->split.buf = nullptr;
+    h->split.launches = 0;
     h->stream = nullptr;
     h->thr = nullptr;
     h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
@@ -243,6 +251,20 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     for (int M = 0; M < 18; ++M) {
         P.cld[M] = -tbit(P.thd.T32, 2 * M - 1);
         P.clp[M] = -tbit(P.thp.T32, 2 * M - 1);
+    }
+    {
+        // Small problems - fewer tile columns than the GPU has warp slots to fill - run each sweep as two kernels:
+        // the state-independent masks of all attempts in parallel, then the sequential update (sweep_warp.cu).
+        // PCPD_SPLIT: unset / "1" auto (at most PCPD_SPLIT_MAX_TASKS tile columns), "0" never, "force" whenever the
+        // mask buffer stays below 1 GiB.
+        const char *sm = getenv("PCPD_SPLIT");
+        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : 1;
+        const uint64_t ntasks = (L / Ts) * W;
+        const size_t bytes = split_mask_bytes(P);
+        if (mode && split_supported(Ts, D) && !h->force_block &&
+            (mode == 2 ? bytes <= (1ull << 30) : ntasks <= PCPD_SPLIT_MAX_TASKS)) {
+            h->split.buf = dev_alloc(bytes, h->stream);   // failure: the fused kernel is used
+        }
     }
     g_err[0] = 0;
     return h;
@@ -305,6 +327,8 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
     }
     h->P.thr_dev = h->thr;
     h->force_block = false;
+    dev_free(h->split.buf);   // per-word thresholds run the fused kernel
+    h->split.buf = nullptr;
     return h;
 }
 
@@ -313,6 +337,7 @@ void pcpd_destroy(pcpd_t *h)
     if (!h) return;
     cudaStreamSynchronize(h->stream);
     dev_free(h->thr);
+    dev_free(h->split.buf);
     dev_free(h->lat);
     dev_free(h->counts);
     delete h;
@@ -348,7 +373,7 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit);
+        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit, &h->split);
         h->sweep += 1;
     }
     return check_launch("sweep kernel");
@@ -448,6 +473,7 @@ int pcpd_synchronize(pcpd_t *h)
 }
 
 int pcpd_jit_state(const pcpd_t *h) { return h ? h->jit.state : 0; }
+uint64_t pcpd_split_launch_count(const pcpd_t *h) { return h ? h->split.launches : 0; }
 const char *pcpd_jit_message(void) { return jit_message(); }
 uint64_t pcpd_jit_launch_count(void) { return jit_launch_count(); }
 

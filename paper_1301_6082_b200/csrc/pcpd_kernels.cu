@@ -194,10 +194,11 @@ static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
 
 // The production path is the warp-per-(tile, column) kernel of sweep_warp.cu; the block kernel
 // above only serves schedules with more than 32 domains per tile.
-int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit)
+int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit,
+                 SplitSlot *split)
 {
     if (sweep_warp_supported(P.Ts, P.D) && !force_block_kernel)
-        return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream, jit);
+        return launch_sweep_warp(P, variant, sweep_warp_wpb(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream, jit, split);
     return variant == 0 ? launch_sweep_t<0>(P, stream) : variant == 1 ? launch_sweep_t<1>(P, stream)
            : variant == 2 ? launch_sweep_t<2>(P, stream) : launch_sweep_t<3>(P, stream);
 }

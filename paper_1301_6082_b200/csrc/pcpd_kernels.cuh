@@ -42,6 +42,11 @@ struct SweepParams {
     const uint32_t *thr_dev;
     uint32_t connected;       // 1: connected multispin lattice: words of tile sites past the ring wrap are bit-rotated (C10)
     uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
+    // SPLIT path (small problems): per (tile column task, attempt of the sweep) three rows of 32 uint4, written by
+    // mask_kernel, read by sweep_warp_kernel<..., SPLIT = 2>; split_nud / split_nup = prefix lengths they hold
+    void *mask_dev;
+    uint32_t split_nud, split_nup;
+    uint32_t rr;              // right reach of the variant's footprint: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
 };
 
 #ifndef __CUDACC_RTC__
@@ -52,12 +57,21 @@ struct JitSlot {
     void *kernel;  // CUfunction
 };
 
+// SPLIT path of one handle (small problems): mask buffer (device; NULL = path not used) and a launch counter.
+struct SplitSlot {
+    void *buf;
+    uint64_t launches;
+};
+size_t split_mask_bytes(const SweepParams &P);
+bool split_supported(uint32_t Ts, uint32_t D);
+
 // Launchers (all asynchronous on `stream`); return the number of kernels launched.
-int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit);
+int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit,
+                 SplitSlot *split);
 // warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);
-int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit);
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split);
 // jit.cu: compile (once per process, device and parameter set)
 // sweep_warp_kernel<variant, wpb, nud, nup, pmode, 0, 1, Td, Tp, Ts, D, A, L> with NVRTC and load it; NULL if NVRTC or the driver entry points are unavailable or the compilation fails
 // (message in jit_message()).  jit_launch returns a cudaError_t-like code (0 = launched).

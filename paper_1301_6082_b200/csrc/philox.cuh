@@ -4,6 +4,7 @@
 #pragma once
 #ifdef __CUDACC_RTC__
 // run-time compilation (jit.cu): no standard headers; NVRTC's own fixed-width built-in types
+typedef unsigned char uint8_t;
 typedef unsigned int uint32_t;
 typedef int int32_t;
 typedef unsigned long long uint64_t;

@@ -76,9 +76,64 @@ static int warp_op_any(int variant, int wpb, int nud, int nup, const SweepParams
     return wpb == 7 ? warp_op_d<1, 7>(nud, nup, P, stream) : warp_op_d<1, 1>(nud, nup, P, stream);
 }
 
-int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit)
+// ---- SPLIT path for small problems: mask_kernel (all attempts of the sweep in parallel) + consumer kernel ----
+// consumer's shared memory: tile buffer, the task's J mask records (TMA bulk copies), one mbarrier per chunk
+static size_t split_smem_bytes(uint32_t Ts, uint32_t J)
+{
+    return ((warp_smem_bytes(Ts, 1) + 127) & ~(size_t)127) + (size_t)J * MASK_REC_BYTES + MASK_MAX_CHUNKS * 8;
+}
+
+bool split_supported(uint32_t Ts, uint32_t D)   // J = S * A = D attempts per domain and sweep
+{
+    return sweep_warp_supported(Ts, D) && D <= MASK_CHUNK * MASK_MAX_CHUNKS && split_smem_bytes(Ts, D) <= 226 * 1024;
+}
+
+template <int VARIANT, int PMODE>
+static int split_consumer_op(const SweepParams *P, cudaStream_t stream)
+{
+    auto kern = sweep_warp_kernel<VARIANT, 1, 0, 0, PMODE, 0, 0, 0u, 0u, 0u, 0u, 0u, 0u, 2>;
+    if (!P) return (int)cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+    kern<<<(P->L / P->Ts) * P->W, 32, split_smem_bytes(P->Ts, P->S * P->A), stream>>>(*P);
+    return 1;
+}
+
+static int split_consumer_any(int variant, int pmode, const SweepParams *P, cudaStream_t stream)
+{
+    switch (variant * 2 + pmode) {
+    case 0: return split_consumer_op<0, 0>(P, stream);
+    case 1: return split_consumer_op<0, 1>(P, stream);
+    case 2: return split_consumer_op<1, 0>(P, stream);
+    case 3: return split_consumer_op<1, 1>(P, stream);
+    case 4: return split_consumer_op<2, 0>(P, stream);
+    case 5: return split_consumer_op<2, 1>(P, stream);
+    case 6: return split_consumer_op<3, 0>(P, stream);
+    default: return split_consumer_op<3, 1>(P, stream);
+    }
+}
+
+size_t split_mask_bytes(const SweepParams &P) { return (size_t)(P.L / P.Ts) * P.W * P.S * P.A * 96u * sizeof(uint4); }
+
+// Small problems (SplitSlot::buf allocated by the API layer when the handle qualifies): two launches per sweep.
+static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t stream, SplitSlot *split)
+{
+    SweepParams P = P0;
+    // prefix lengths: up to 8 blocks per stream - the producer is parallel over all attempts of the sweep, and every
+    // tail iteration it saves the consumer is ~150 cycles on the sequential chain
+    P.mask_dev = split->buf;
+    P.split_nud = min((P.thd.nplanes + 1u) >> 1, 8u);
+    P.split_nup = P.pmask_paper ? 1u : min((P.thp.nplanes + 1u) >> 1, 8u);
+    P.rr = variant == 3 ? 1u : 2u + (uint32_t)variant;
+    const uint32_t nwarps = (P.L / P.Ts) * P.W * P.S * P.A;
+    mask_kernel<<<(nwarps + 3) / 4, 128, 0, stream>>>(P);
+    split_consumer_any(variant, P.pmask_paper ? 1 : 0, &P, stream);
+    split->launches += 2;
+    return 2;
+}
+
+int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split)
 {
     if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
+    if (split && split->buf && !(jit && jit->mode == 2)) return launch_sweep_split(P, variant, stream, split);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
     const int nud = nu_d_of((P.thd.nplanes + 1) >> 1);
     // Threshold-specialised kernel (jit.cu): large problems (wpb == 7), or every size with PCPD_JIT=force.  Not
@@ -119,6 +174,11 @@ int configure_warp_kernels()
                     if (e != 0) return e;
                 }
             const int e = warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, nullptr, nullptr);
+            if (e != 0) return e;
+        }
+    for (int variant = 0; variant < 4; ++variant)
+        for (int pmode = 0; pmode < 2; ++pmode) {
+            const int e = split_consumer_any(variant, pmode, nullptr, nullptr);
             if (e != 0) return e;
         }
     return 0;

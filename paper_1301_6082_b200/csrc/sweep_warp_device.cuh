@@ -176,6 +176,69 @@ __device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &b
     cmp2h_sum(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1, s0, s1);
 }
 
+// ---- TMA bulk copy + mbarrier (SPLIT consumer: the task's mask records are staged through shared memory) ----
+constexpr uint32_t MASK_REC_BYTES = 96u * 16u;  // one attempt: three rows of 32 uint4
+constexpr uint32_t MASK_CHUNK = 4u;             // attempts per bulk copy / mbarrier
+constexpr uint32_t MASK_MAX_CHUNKS = 64u;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!done);
+}
+
+// C5 step 3-4 for domain b in a sub-step with inner shift sigma: only domain n-1 with sigma > 0 wraps; the tile
+// seam lies between domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
+struct DomainPos {
+    int32_t lo, rem;
+    uint32_t n_allow, dbase;  // dbase = tile-local index of domain-local 0 (before wrap)
+};
+__device__ __forceinline__ DomainPos domain_pos(uint32_t b, uint32_t n, uint32_t sigma, uint32_t D, uint32_t Rr)
+{
+    DomainPos dp;
+    const bool seam = (b == n - 1) && (sigma > 0);
+    const int32_t c = (int32_t)D - (int32_t)sigma;
+    dp.lo = 0;
+    dp.rem = 0;
+    if (seam) {
+        dp.lo = max(1, c - (int32_t)Rr);
+        const int32_t hi = min((int32_t)D - 1 - (int32_t)Rr, c);
+        dp.rem = max(0, hi - dp.lo + 1);
+    }
+    dp.n_allow = D - 1 - Rr - (uint32_t)dp.rem;
+    dp.dbase = sigma + b * D;
+    return dp;
+}
+// C4 / C5 step 4: position selector x2 of the MISC block -> tile-local index of footprint site x-1
+__device__ __forceinline__ uint32_t footprint_start(uint32_t x2, const DomainPos &dp, uint32_t Ts)
+{
+    int32_t x = 1 + (int32_t)__umulhi(x2, dp.n_allow);
+    if (dp.rem > 0 && x >= dp.lo) x += dp.rem;
+    uint32_t y0 = dp.dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
+    if (y0 >= Ts) y0 -= Ts;
+    return y0;
+}
+
 // blocks of a threshold T in [0, 2^32): ceil((32 - ctz(T)) / 2), 0 for T = 0
 __host__ __device__ constexpr uint32_t nblk_of(uint32_t T)
 {
@@ -218,8 +281,15 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
 // SPEC = 1 (kernels compiled at run time by jit.cu): the thresholds are the template constants STD, STP
 // (low 32 bits of T_d, T_p; neither threshold is 2^32) instead of P.thd / P.thp and the host tables, and
 // the schedule constants T_s, D, A and the ring length L are the template constants CTS, CD, CA, CL.
+//
+// SPLIT = 2 (small problems, too few tile columns to fill the GPU): the state-independent part of every
+// attempt - MISC block and the compared prefix planes of DIFF and ANNI - has been computed for the whole
+// sweep by mask_kernel below, in parallel over all attempts, into P.mask_dev; this kernel then only reads
+// them (prefetched one attempt ahead), so that the sequential chain of a domain's D attempts per sweep is
+// ~150 cycles per attempt instead of ~1400.  Prefix lengths are then the run-time values P.split_nud /
+// P.split_nup (NU_D, NU_P unused).  Same results bit for bit.
 template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW, int SPEC = 0, uint32_t STD = 0u, uint32_t STP = 0u,
-          uint32_t CTS = 0u, uint32_t CD = 0u, uint32_t CA = 0u, uint32_t CL = 0u>
+          uint32_t CTS = 0u, uint32_t CD = 0u, uint32_t CA = 0u, uint32_t CL = 0u, int SPLIT = 0>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
@@ -319,45 +389,74 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 
+    // SPLIT consumer (WPB = 1): the records of this task's J = S*A attempts (three rows of 32 uint4 each, contiguous
+    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies of MASK_CHUNK attempts,
+    // each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a chunk only when it
+    // reaches its first attempt, and reads each record one attempt ahead of its use.
+    const uint32_t nud = SPLIT == 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT == 2 ? P.split_nup : (uint32_t)NU_P;
+    const uint4 *mrec = nullptr;
+    uint64_t *bars = nullptr;
+    uint4 nx0{}, nx1{}, nx2{};
+    if constexpr (SPLIT == 2) {
+        const uint32_t J = S * A, nch = (J + MASK_CHUNK - 1u) / MASK_CHUNK;
+        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
+        bars = reinterpret_cast<uint64_t *>(mbase + (size_t)J * MASK_REC_BYTES);
+        if (lane == 0) {
+            for (uint32_t c = 0; c < nch; ++c) mbar_init(bars + c, 1u);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            const uint8_t *src = reinterpret_cast<const uint8_t *>(P.mask_dev) + (size_t)task * J * MASK_REC_BYTES;
+            for (uint32_t c = 0; c < nch; ++c) {
+                const uint32_t j0 = c * MASK_CHUNK, bytes = (min(j0 + MASK_CHUNK, J) - j0) * MASK_REC_BYTES;
+                mbar_expect_tx(bars + c, bytes);
+                bulk_g2s(mbase + (size_t)j0 * MASK_REC_BYTES, src + (size_t)j0 * MASK_REC_BYTES, bytes, bars + c);
+            }
+        }
+        __syncwarp();
+        mrec = reinterpret_cast<const uint4 *>(mbase) + lane;
+        mbar_wait(bars, 0u);
+        nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64];
+    }
 #pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
-        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
-        const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
-        // C5 step 3-4: only domain n-1 with sigma > 0 wraps; seam between
-        // domain-local c-1 and c, c = D - sigma; positions [c-Rr, c] are excluded.
-        const bool seam = (b == n - 1) && (sigma > 0);
-        const int32_t c = (int32_t)D - (int32_t)sigma;
-        int32_t lo = 0, rem = 0;
-        if (seam) {
-            lo = max(1, c - (int32_t)Rr);
-            const int32_t hi = min((int32_t)D - 1 - (int32_t)Rr, c);
-            rem = max(0, hi - lo + 1);
+        DomainPos dp{};
+        if constexpr (SPLIT != 2) {  // (SPLIT consumer: mask_kernel has resolved the positions)
+            if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
+            const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
+            dp = domain_pos(b, n, sigma, D, Rr);
         }
-        const uint32_t n_allow = D - 1 - Rr - (uint32_t)rem;
-        const uint32_t dbase = sigma + b * D;  // tile-local index of domain-local 0 (before wrap)
 
 #pragma unroll 1
         for (uint32_t a = 0; a < A; ++a) {
             // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
             // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
             // back to back so that the FMA pipe always has several wide multiplies in flight.
-            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
-            uint32_t c3s[1 + NU_D + NU_P];
+            PhiloxSlot ps{};
+            if constexpr (SPLIT != 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
             U4 blks[1 + NU_D + NU_P];
-            c3s[0] = STREAM_MISC;
+            Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
+            if constexpr (SPLIT == 2) {
+                // this attempt's record was fetched during the previous attempt; fetch the next one now
+                const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
+                const uint32_t jn = min(k * A + a + 1u, S * A - 1u);
+                if (jn % MASK_CHUNK == 0u) mbar_wait(bars + jn / MASK_CHUNK, 0u);
+                nx0 = mrec[jn * 96u]; nx1 = mrec[jn * 96u + 32u]; nx2 = mrec[jn * 96u + 64u];
+                blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
+                dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
+                plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
+            } else {
+                uint32_t c3s[1 + NU_D + NU_P];
+                c3s[0] = STREAM_MISC;
 #pragma unroll
-            for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
+                for (int m = 0; m < NU_D; ++m) c3s[1 + m] = STREAM_DIFF | m;
 #pragma unroll
-            for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
-            philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, rk, blks);
+                for (int m = 0; m < NU_P; ++m) c3s[1 + NU_D + m] = STREAM_ANNI | m;
+                philox_blocks<1 + NU_D + NU_P>(c3s, ps, pw, rk, blks);
+            }
             const U4 misc = blks[0];
             const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
 
             // C4: MISC block: Fm = ~lo (1 -> fission low, Alg. 1: r3 < 1/2), x2 -> position.
-            int32_t x = 1 + (int32_t)__umulhi(misc.x2, n_allow);
-            if (rem > 0 && x >= lo) x += rem;
-            uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
-            if (y0 >= Ts) y0 -= Ts;
+            const uint32_t y0 = SPLIT == 2 ? misc.x2 : footprint_start(misc.x2, dp, Ts);  // (SPLIT: resolved by mask_kernel)
             const uint64_t Fm = ~lo64(misc);
             uint64_t *q = tile + y0;
             uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0, sg = 0;
@@ -371,8 +470,9 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
             // dependence on the state), the lazy tails only on the lanes whose outcome can matter:
             // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
-            Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-            if constexpr (SPEC) {
+            if constexpr (SPLIT == 2) {
+                // prefix compared by mask_kernel
+            } else if constexpr (SPEC) {
                 prefix_spec<STD, NU_D>(dlt, dund, dblk);
                 if constexpr (PMODE == 0) prefix_spec<STP, NU_P>(plt, pund, pblk);
             } else {
@@ -392,11 +492,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 const uint64_t rel = sb | sc;
                 dund.lo &= (uint32_t)rel;
                 dund.hi &= (uint32_t)(rel >> 32);
-                uint32_t Tsh = Td << (2 * NU_D);  // T's bits of the next two planes on top (0 past the last plane)
-                uint32_t m = NU_D;
+                uint32_t Tsh = Td << (2 * nud);  // T's bits of the next two planes on top (0 past the last plane)
+                uint32_t m = nud;
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
+                    if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -421,10 +522,11 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             if constexpr (PMODE == 0) {
                 pund.lo &= (uint32_t)react;
                 pund.hi &= (uint32_t)(react >> 32);
-                uint32_t Tsh = Tp << (2 * NU_P);
-                uint32_t m = NU_P;
+                uint32_t Tsh = Tp << (2 * nup);
+                uint32_t m = nup;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
+                    if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -443,9 +545,11 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
                 // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
                 // word-wide draw that is 1 w.p. 4p (x3 of the MISC block against floor(4p * 2^32)).
-                const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-                plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
-                plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
+                if constexpr (SPLIT != 2) {  // (SPLIT consumer: mask_kernel has done this)
+                    const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
+                    plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
+                    plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
+                }
             }
             const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);
 
@@ -512,6 +616,49 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             g[i] = tile[y];
         }
     }
+}
+
+// mask_kernel - producer of the SPLIT path: one warp per (tile column task, attempt j of the sweep); lane = domain.
+// Computes everything of an attempt that does not depend on the lattice: the MISC block (fission-side mask and the
+// footprint position, resolved to the tile-local index of site x-1 with the sub-step's inner shift and seam), and the
+// generic-threshold compare of the first P.split_nud DIFF and P.split_nup ANNI blocks (the paper's gated mask when
+// P.pmask_paper), and stores them as three coalesced uint4 rows per attempt: {misc x0, x1, y0, x3}, {dlt, dund},
+// {plt, pund}.  The blocks of a warp are evaluated one after the other (run-time loop): the parallelism is across the
+// (L / T_s) * W * D warps of the grid.
+__global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ SweepParams P)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t J = P.S * P.A, ntiles = P.L / P.Ts;
+    const uint32_t gw = blockIdx.x * 4u + (threadIdx.x >> 5);
+    if (gw >= ntiles * P.W * J) return;
+    const uint32_t task = gw / J, j = gw - task * J;
+    const uint32_t tau = task % ntiles, wl = task / ntiles;
+    const uint32_t b = lane < P.n ? lane : 0u;
+    const RoundKeys &rk = P.rk;
+    const uint32_t sigma = __umulhi(philox4x32_10(j / P.A, P.t, 0u, STREAM_SHIFT, rk).x0, P.D);  // C5 step 1
+    const DomainPos dp = domain_pos(b, P.n, sigma, P.D, P.rr);
+    const PhiloxWarp pw = philox_warp_consts(P.t, P.word_offset + wl, rk);
+    const PhiloxSlot ps = philox_slot_consts((tau * P.n + b) * P.D + j, pw, rk);
+    const U4 misc = philox_block(STREAM_MISC, ps, pw, rk);
+    const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
+    Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
+    for (uint32_t m = 0; m < P.split_nud; ++m)
+        cmp_block_sum(dlt, dund, philox_block(STREAM_DIFF | m, ps, pw, rk), P.tdm[2 * m], P.tdm[2 * m + 1], P.sd[2 * m],
+                      P.sd[2 * m + 1]);
+    if (!P.pmask_paper) {
+        for (uint32_t m = 0; m < P.split_nup; ++m)
+            cmp_block_sum(plt, pund, philox_block(STREAM_ANNI | m, ps, pw, rk), P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m],
+                          P.sp[2 * m + 1]);
+    } else {
+        const U4 pb = philox_block(STREAM_ANNI, ps, pw, rk);
+        const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
+        plt.lo = pb.x0 & pb.x2 & gate;
+        plt.hi = pb.x1 & pb.x3 & gate;
+    }
+    uint4 *rec = reinterpret_cast<uint4 *>(P.mask_dev) + (size_t)gw * 96u + lane;
+    rec[0] = make_uint4(misc.x0, misc.x1, y0, misc.x3);
+    rec[32] = make_uint4(dlt.lo, dlt.hi, dund.lo, dund.hi);
+    rec[64] = make_uint4(plt.lo, plt.hi, pund.lo, pund.hi);
 }
 
 }  // namespace pcpd

@@ -55,7 +55,7 @@ def oracle_columns(cfg_kw, words, init, n_sweeps_list, words_in=None):
     return out
 
 
-def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=False):
+def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=False, expect_split=None):
     W = kw["n_replicas"] // 64
     words = list(range(W)) if words is None else words
     okw = dict(kw)
@@ -82,6 +82,8 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
     assert g.sweep == times[-1]
     if expect_jit:  # the sweeps ran the threshold-specialised (run-time compiled) kernel, not the built-in one
         assert g.jit_state() == 1, pk.jit_message()
+    if expect_split is not None:  # two-kernel small-problem path (mask_kernel + update kernel) or the fused kernel
+        assert g.split_launch_count() == (2 * times[-1] if expect_split else 0)
     g.close()
 
 
@@ -130,11 +132,18 @@ SMALL = [
 ]
 
 
+@pytest.mark.parametrize("split", ["auto", "0"])
 @pytest.mark.parametrize("case", SMALL, ids=[f"case{i}" for i in range(len(SMALL))])
-def test_small_cases_bit_exact_every_sweep(pk, case):
+def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
+    """Every word and count after every sweep.  split = auto: these sizes run the two-kernel small-problem path
+    (mask_kernel + update kernel) wherever the warp kernel applies (at most 32 domains per tile); split = 0: the
+    fused warp kernel (or the block kernel for more than 32 domains per tile)."""
     variant, L, R, d, p, Ts, D, A, init = case
+    if split == "0":
+        monkeypatch.setenv("PCPD_SPLIT", "0")
     kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
-    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)))
+    warp = min(Ts, L) // D <= 32
+    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)), expect_split=(split == "auto" and warp))
 
 
 # cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
