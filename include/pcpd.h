@@ -189,9 +189,10 @@ PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t
  * the machine idle and each sweep is the latency of one warp's chain of D attempts.  Such handles (at most 592
  * tile columns by default) run each sweep as two launches: mask_kernel computes the state-independent part of
  * ALL attempts of the sweep in parallel (MISC block, compared prefix planes of DIFF and ANNI), then the update
- * kernel reads them and applies the attempts in order.  Same results bit for bit.  Environment, read by
+ * kernel reads them and applies the attempts in order; the masks do not depend on the lattice, so those of
+ * sweep t+1 are computed on an internal auxiliary stream while sweep t is applied.  Same results bit for bit.  Environment, read by
  * pcpd_create*: PCPD_SPLIT=0 never; PCPD_SPLIT=force whenever the mask buffer stays below 1 GiB (test hook).
- * pcpd_split_launch_count: kernels this handle has launched on that path (2 per sweep; 0 = fused kernel). */
+ * pcpd_split_launch_count: kernels this handle has launched on that path (2 per sweep + 1; 0 = fused kernel). */
 PCPD_API uint64_t pcpd_split_launch_count(const pcpd_t *h);
 
 /* Number of kernels this library has launched so far in this process. */

@@ -216,8 +216,7 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         h->jit.state = 0;
         h->jit.kernel = nullptr;
     }
-    h->split.buf = nullptr;
-    h->split.launches = 0;
+    memset(&h->split, 0, sizeof h->split);
     h->stream = nullptr;
     h->thr = nullptr;
     h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
@@ -263,7 +262,15 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         const size_t bytes = split_mask_bytes(P);
         if (mode && split_supported(Ts, D) && !h->force_block &&
             (mode == 2 ? bytes <= (1ull << 30) : ntasks <= PCPD_SPLIT_MAX_TASKS)) {
-            h->split.buf = dev_alloc(bytes, h->stream);   // failure: the fused kernel is used
+            h->split.buf[0] = dev_alloc(bytes, h->stream);   // any failure here: the fused kernel is used
+            h->split.buf[1] = h->split.buf[0] ? dev_alloc(bytes, h->stream) : nullptr;
+            if (!h->split.buf[1] || split_setup(&h->split) != 0) {
+                cudaGetLastError();
+                split_teardown(&h->split);
+                dev_free(h->split.buf[0]);
+                dev_free(h->split.buf[1]);
+                h->split.buf[0] = h->split.buf[1] = nullptr;
+            }
         }
     }
     g_err[0] = 0;
@@ -327,8 +334,10 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
     }
     h->P.thr_dev = h->thr;
     h->force_block = false;
-    dev_free(h->split.buf);   // per-word thresholds run the fused kernel
-    h->split.buf = nullptr;
+    split_teardown(&h->split);   // per-word thresholds run the fused kernel
+    dev_free(h->split.buf[0]);
+    dev_free(h->split.buf[1]);
+    h->split.buf[0] = h->split.buf[1] = nullptr;
     return h;
 }
 
@@ -336,8 +345,10 @@ void pcpd_destroy(pcpd_t *h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
+    split_teardown(&h->split);
     dev_free(h->thr);
-    dev_free(h->split.buf);
+    dev_free(h->split.buf[0]);
+    dev_free(h->split.buf[1]);
     dev_free(h->lat);
     dev_free(h->counts);
     delete h;

@@ -57,11 +57,20 @@ struct JitSlot {
     void *kernel;  // CUfunction
 };
 
-// SPLIT path of one handle (small problems): mask buffer (device; NULL = path not used) and a launch counter.
+// SPLIT path of one handle (small problems).  The masks of a sweep depend on (seed, t, schedule, thresholds) only, not
+// on the lattice, so mask_kernel(t + 1) runs on an auxiliary stream while the update kernel of sweep t runs on the
+// handle's stream: two mask buffers (buf[t & 1]), `held[i]` = the sweep whose masks buf[i] holds (or will hold once
+// ready[i] fires), freed[i] = the update kernel that last read buf[i] has finished.
 struct SplitSlot {
-    void *buf;
+    void *buf[2];          // device; buf[0] == NULL: path not used
     uint64_t launches;
+    cudaStream_t aux;
+    cudaEvent_t ready[2], freed[2];
+    int64_t held[2];       // -1: nothing
+    bool freed_valid[2];
 };
+int split_setup(SplitSlot *s);     // creates the stream and events (buffers are allocated by the API layer); 0 = ok
+void split_teardown(SplitSlot *s);
 size_t split_mask_bytes(const SweepParams &P);
 bool split_supported(uint32_t Ts, uint32_t D);
 

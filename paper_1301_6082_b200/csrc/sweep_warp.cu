@@ -114,26 +114,78 @@ static int split_consumer_any(int variant, int pmode, const SweepParams *P, cuda
 size_t split_mask_bytes(const SweepParams &P) { return (size_t)(P.L / P.Ts) * P.W * P.S * P.A * 96u * sizeof(uint4); }
 
 // Small problems (SplitSlot::buf allocated by the API layer when the handle qualifies): two launches per sweep.
+int split_setup(SplitSlot *s)
+{
+    if (cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking) != cudaSuccess) return -1;
+    for (int i = 0; i < 2; ++i) {
+        if (cudaEventCreateWithFlags(&s->ready[i], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&s->freed[i], cudaEventDisableTiming) != cudaSuccess)
+            return -1;
+        s->held[i] = -1;
+        s->freed_valid[i] = false;
+    }
+    return 0;
+}
+
+void split_teardown(SplitSlot *s)
+{
+    if (!s->aux) return;
+    cudaStreamSynchronize(s->aux);
+    for (int i = 0; i < 2; ++i) {
+        if (s->ready[i]) cudaEventDestroy(s->ready[i]);
+        if (s->freed[i]) cudaEventDestroy(s->freed[i]);
+    }
+    cudaStreamDestroy(s->aux);
+    s->aux = nullptr;
+}
+
+// masks of sweep t into buf[t & 1], on the auxiliary stream, once the last reader of that buffer has finished
+static void split_produce(const SweepParams &P, uint32_t t, SplitSlot *split)
+{
+    const int i = (int)(t & 1u);
+    SweepParams Q = P;
+    Q.t = t;
+    Q.mask_dev = split->buf[i];
+    if (split->freed_valid[i]) cudaStreamWaitEvent(split->aux, split->freed[i], 0);
+    const uint32_t nwarps = (Q.L / Q.Ts) * Q.W * Q.S * Q.A;
+    mask_kernel<<<(nwarps + 3) / 4, 128, 0, split->aux>>>(Q);
+    cudaEventRecord(split->ready[i], split->aux);
+    split->held[i] = (int64_t)t;
+}
+
+// Small problems: two launches per sweep; the masks of sweep t + 1 are produced while sweep t is applied.
 static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t stream, SplitSlot *split)
 {
     SweepParams P = P0;
     // prefix lengths: up to 8 blocks per stream - the producer is parallel over all attempts of the sweep, and every
     // tail iteration it saves the consumer is ~150 cycles on the sequential chain
-    P.mask_dev = split->buf;
     P.split_nud = min((P.thd.nplanes + 1u) >> 1, 8u);
     P.split_nup = P.pmask_paper ? 1u : min((P.thp.nplanes + 1u) >> 1, 8u);
     P.rr = variant == 3 ? 1u : 2u + (uint32_t)variant;
-    const uint32_t nwarps = (P.L / P.Ts) * P.W * P.S * P.A;
-    mask_kernel<<<(nwarps + 3) / 4, 128, 0, stream>>>(P);
+    const uint32_t t = P.t;
+    const int i = (int)(t & 1u);
+    int launched = 1;
+    if (split->held[i] != (int64_t)t) {   // not prefetched (first sweep of the handle, or the counter was set)
+        split_produce(P, t, split);
+        ++launched;
+    }
+    if (t != 0xffffffffu && split->held[i ^ 1] != (int64_t)t + 1) {
+        split_produce(P, t + 1u, split);
+        ++launched;
+    }
+    cudaStreamWaitEvent(stream, split->ready[i], 0);
+    P.mask_dev = split->buf[i];
     split_consumer_any(variant, P.pmask_paper ? 1 : 0, &P, stream);
-    split->launches += 2;
-    return 2;
+    cudaEventRecord(split->freed[i], stream);
+    split->freed_valid[i] = true;
+    split->launches += (uint64_t)launched;
+    return launched;
 }
 
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split)
 {
     if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
-    if (split && split->buf && !(jit && jit->mode == 2)) return launch_sweep_split(P, variant, stream, split);
+    if (split && split->buf[0] && !(jit && jit->mode == 2)) return launch_sweep_split(P, variant, stream, split);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
     const int nud = nu_d_of((P.thd.nplanes + 1) >> 1);
     // Threshold-specialised kernel (jit.cu): large problems (wpb == 7), or every size with PCPD_JIT=force.  Not

@@ -83,7 +83,8 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
     if expect_jit:  # the sweeps ran the threshold-specialised (run-time compiled) kernel, not the built-in one
         assert g.jit_state() == 1, pk.jit_message()
     if expect_split is not None:  # two-kernel small-problem path (mask_kernel + update kernel) or the fused kernel
-        assert g.split_launch_count() == (2 * times[-1] if expect_split else 0)
+        # (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being launched one sweep ahead)
+        assert g.split_launch_count() == (2 * times[-1] + 1 if expect_split else 0)
     g.close()
 
 
