@@ -85,7 +85,7 @@ static size_t split_smem_bytes(uint32_t Ts, uint32_t J)
 
 bool split_supported(uint32_t Ts, uint32_t D)   // J = S * A = D attempts per domain and sweep
 {
-    return sweep_warp_supported(Ts, D) && D <= MASK_CHUNK * MASK_MAX_CHUNKS && split_smem_bytes(Ts, D) <= 226 * 1024;
+    return sweep_warp_supported(Ts, D) && split_smem_bytes(Ts, D) <= 226 * 1024;
 }
 
 template <int VARIANT, int PMODE>

@@ -178,8 +178,7 @@ __device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &b
 
 // ---- TMA bulk copy + mbarrier (SPLIT consumer: the task's mask records are staged through shared memory) ----
 constexpr uint32_t MASK_REC_BYTES = 96u * 16u;  // one attempt: three rows of 32 uint4
-constexpr uint32_t MASK_CHUNK = 4u;             // attempts per bulk copy / mbarrier
-constexpr uint32_t MASK_MAX_CHUNKS = 64u;
+constexpr uint32_t MASK_MAX_CHUNKS = 256u;      // one bulk copy / mbarrier per sub-step (S <= MAX_SUBSTEPS = 256)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
@@ -390,35 +389,36 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     }
 
     // SPLIT consumer (WPB = 1): the records of this task's J = S*A attempts (three rows of 32 uint4 each, contiguous
-    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies of MASK_CHUNK attempts,
-    // each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a chunk only when it
-    // reaches its first attempt, and reads each record one attempt ahead of its use.
+    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies, one per sub-step (A
+    // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
+    // records when it gets there, and reads each record one attempt ahead of its use.
     const uint32_t nud = SPLIT == 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT == 2 ? P.split_nup : (uint32_t)NU_P;
     const uint4 *mrec = nullptr;
     uint64_t *bars = nullptr;
     uint4 nx0{}, nx1{}, nx2{};
     if constexpr (SPLIT == 2) {
-        const uint32_t J = S * A, nch = (J + MASK_CHUNK - 1u) / MASK_CHUNK;
+        const uint32_t J = S * A, cbytes = A * MASK_REC_BYTES;
         uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
         bars = reinterpret_cast<uint64_t *>(mbase + (size_t)J * MASK_REC_BYTES);
         if (lane == 0) {
-            for (uint32_t c = 0; c < nch; ++c) mbar_init(bars + c, 1u);
+            for (uint32_t c = 0; c < S; ++c) mbar_init(bars + c, 1u);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             const uint8_t *src = reinterpret_cast<const uint8_t *>(P.mask_dev) + (size_t)task * J * MASK_REC_BYTES;
-            for (uint32_t c = 0; c < nch; ++c) {
-                const uint32_t j0 = c * MASK_CHUNK, bytes = (min(j0 + MASK_CHUNK, J) - j0) * MASK_REC_BYTES;
-                mbar_expect_tx(bars + c, bytes);
-                bulk_g2s(mbase + (size_t)j0 * MASK_REC_BYTES, src + (size_t)j0 * MASK_REC_BYTES, bytes, bars + c);
+            for (uint32_t c = 0; c < S; ++c) {
+                mbar_expect_tx(bars + c, cbytes);
+                bulk_g2s(mbase + (size_t)c * cbytes, src + (size_t)c * cbytes, cbytes, bars + c);
             }
         }
         __syncwarp();
         mrec = reinterpret_cast<const uint4 *>(mbase) + lane;
-        mbar_wait(bars, 0u);
-        nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64];
     }
 #pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
         DomainPos dp{};
+        if constexpr (SPLIT == 2) {  // this sub-step's records have landed? then fetch its first one
+            mbar_wait(bars + k, 0u);
+            nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64];
+        }
         if constexpr (SPLIT != 2) {  // (SPLIT consumer: mask_kernel has resolved the positions)
             if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
             const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
@@ -435,11 +435,10 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             U4 blks[1 + NU_D + NU_P];
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
             if constexpr (SPLIT == 2) {
-                // this attempt's record was fetched during the previous attempt; fetch the next one now
+                // this attempt's record was fetched during the previous attempt; fetch the next one of the sub-step now
                 const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
-                const uint32_t jn = min(k * A + a + 1u, S * A - 1u);
-                if (jn % MASK_CHUNK == 0u) mbar_wait(bars + jn / MASK_CHUNK, 0u);
-                nx0 = mrec[jn * 96u]; nx1 = mrec[jn * 96u + 32u]; nx2 = mrec[jn * 96u + 64u];
+                mrec += 96;
+                if (a + 1u < A) { nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64]; }
                 blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
                 dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
                 plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
