@@ -332,6 +332,8 @@ def ours_arm(args, cfg: wl.Config) -> None:
         roof = dict(bound="alu", achieved=achieved / 1e12, peak=mix_peak / 1e12, unit="Tinstr/s",
                     frac=achieved / mix_peak, traffic=NCU_TRAFFIC_BYTES.get(cfg.name),
                     kernel="sweep_warp_kernel" + (" (run-time specialised on T_d, T_p: csrc/jit.cu)" if h.jit_state() == 1
+                                                  else " (update kernel of the two-kernel small-problem path; launch_ms is "
+                                                       "mask_kernel + update kernel per sweep)" if h.split_launch_count() > 0
                                                   else " (built-in generic-threshold kernel)"),
                     launch_ms=sweep_ms,
                     instr_per_attempt_word=alg["lazy"], lazy_blocks=alg["lazy_blocks"],

@@ -186,8 +186,8 @@ PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t
 
 /* ---- small problems: two kernels per sweep -----------
  * With fewer tile columns ((L / T_s) * W) than the GPU has warp slots to fill, one warp per tile column leaves
- * the machine idle and each sweep is the latency of one warp's chain of D attempts.  Such handles (at most 592
- * tile columns by default) run each sweep as two launches: mask_kernel computes the state-independent part of
+ * the machine idle and each sweep is the latency of one warp's chain of D attempts.  Such handles (at most one
+ * tile column per SM) run each sweep as two launches: mask_kernel computes the state-independent part of
  * ALL attempts of the sweep in parallel (MISC block, compared prefix planes of DIFF and ANNI), then the update
  * kernel reads them and applies the attempts in order; the masks do not depend on the lattice, so those of
  * sweep t+1 are computed on an internal auxiliary stream while sweep t is applied.  Same results bit for bit.  Environment, read by

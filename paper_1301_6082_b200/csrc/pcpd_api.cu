@@ -14,11 +14,6 @@
 
 using namespace pcpd;
 
-// SPLIT path (small problems): largest number of tile columns it is used for by default (tuned on B200)
-#ifndef PCPD_SPLIT_MAX_TASKS
-#define PCPD_SPLIT_MAX_TASKS 592u
-#endif
-
 namespace {
 
 thread_local char g_err[512] = "";
@@ -254,14 +249,16 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     {
         // Small problems - fewer tile columns than the GPU has warp slots to fill - run each sweep as two kernels:
         // the state-independent masks of all attempts in parallel, then the sequential update (sweep_warp.cu).
-        // PCPD_SPLIT: unset / "1" auto (at most PCPD_SPLIT_MAX_TASKS tile columns), "0" never, "force" whenever the
-        // mask buffer stays below 1 GiB.
+        // PCPD_SPLIT: unset / "1" auto - at most one tile column per SM: the update kernel keeps a tile column and its
+        // 96 KB of mask records in shared memory, one block per SM, so a second wave doubles its time (measured on
+        // B200 at L = 65536: 128 columns 75 -> 38 us per sweep, 256 columns 76 -> 70 us, 512 columns 76 -> 140 us);
+        // "0" never; "force" whenever the mask buffer stays below 1 GiB.
         const char *sm = getenv("PCPD_SPLIT");
         const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : 1;
         const uint64_t ntasks = (L / Ts) * W;
         const size_t bytes = split_mask_bytes(P);
         if (mode && split_supported(Ts, D) && !h->force_block &&
-            (mode == 2 ? bytes <= (1ull << 30) : ntasks <= PCPD_SPLIT_MAX_TASKS)) {
+            (mode == 2 ? bytes <= (1ull << 30) : ntasks <= (uint64_t)prop.multiProcessorCount)) {
             h->split.buf[0] = dev_alloc(bytes, h->stream);   // any failure here: the fused kernel is used
             h->split.buf[1] = h->split.buf[0] ? dev_alloc(bytes, h->stream) : nullptr;
             if (!h->split.buf[1] || split_setup(&h->split) != 0) {
