@@ -81,6 +81,9 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
             assert np.array_equal(bits.sum(axis=0).ravel().astype(np.uint32), cnt)
     assert g.sweep == times[-1]
     if expect_jit:  # the sweeps ran the threshold-specialised (run-time compiled) kernel, not the built-in one
+        if g.jit_state() != 1 and "libnvrtc not found" in pk.jit_message():
+            g.close()
+            pytest.skip("libnvrtc is not installed on this box: the built-in kernel ran (and passed the checks above)")
         assert g.jit_state() == 1, pk.jit_message()
     if expect_split is not None:  # two-kernel small-problem path (mask_kernel + update kernel) or the fused kernel
         # (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being launched one sweep ahead)
@@ -174,6 +177,9 @@ def test_specialised_and_builtin_kernels_agree_at_full_size(pk, monkeypatch):
             g = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
             g.init(c.init)
             g.run(3)
+            if mode == "1" and g.jit_state() != 1 and "libnvrtc not found" in pk.jit_message():
+                g.close()
+                pytest.skip("libnvrtc is not installed on this box")
             assert g.jit_state() == (1 if mode == "1" else 0), pk.jit_message()
             res.append((g.get_lattice(), g.density()))
             g.close()
@@ -226,6 +232,30 @@ def test_invariants_on_gpu(pk):
     assert np.array_equal(a.get_lattice(), c.get_lattice())
     for h in (a, b, c):
         h.close()
+
+
+def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
+    """The two-kernel small-problem path produces the masks of sweep t+1 one sweep ahead on an auxiliary stream
+    (double-buffered).  Re-initialising, and setting the sweep counter backwards, forwards or to the value already
+    prefetched, must give what the fused kernel gives for the same sequence of calls."""
+    def sequence(g):
+        out = []
+        g.init(1); g.run(3); out.append(g.get_lattice())
+        g.init(1); g.run(2); out.append(g.get_lattice())      # counter back to 0 with stale prefetched masks
+        g.sweep = 9; g.run(1); g.run(2); out.append(g.get_lattice())
+        g.sweep = 12; g.run(1); out.append(g.get_lattice())   # counter set to the sweep whose masks are already there
+        g.sweep = 4; g.run(3); out.append(g.get_lattice())
+        g.sweep = 2 ** 32 - 2; g.run(1); out.append(g.get_lattice())   # last legal sweep: nothing to prefetch
+        return out
+    res = []
+    for mode in ("1", "0"):
+        monkeypatch.setenv("PCPD_SPLIT", mode)
+        g = pk.Pcpd(4096, 192, 0.3, 0.12, 11, 0)
+        res.append(sequence(g))
+        assert (g.split_launch_count() > 0) == (mode == "1")
+        g.close()
+    for x, y in zip(*res):
+        assert np.array_equal(x, y)
 
 
 def test_word_offset_shards_equal_one_big_run(pk):
