@@ -35,7 +35,7 @@ import workloads as wl
 SWEEPS_PER_STEP = 10
 # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch from the committed `ncu --set full` capture
 # (profiles/), per config; None where no capture exists.
-NCU_TRAFFIC_BYTES = {"cfg4": 2.090e9}   # profiles/r1b_sweep_kernel_full.md
+NCU_TRAFFIC_BYTES = {"cfg4": 2.091e9}   # profiles/r1d_sweep_kernel_full.md (1.075 GB read + 1.016 GB written per launch)
 METRIC = "replica_site_updates_per_sec"
 UNIT = "replica-site updates/s"
 

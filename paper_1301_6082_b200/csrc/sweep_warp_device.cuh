@@ -623,7 +623,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
 // generic-threshold compare of the first P.split_nud DIFF and P.split_nup ANNI blocks (the paper's gated mask when
 // P.pmask_paper), and stores them as three coalesced uint4 rows per attempt: {misc x0, x1, y0, x3}, {dlt, dund},
 // {plt, pund}.  The blocks of a warp are evaluated one after the other (run-time loop): the parallelism is across the
-// (L / T_s) * W * D warps of the grid.
+// (L / T_s) * W * D warps of the grid.  (Not part of the run-time specialised build, which is for large problems.)
+#ifndef PCPD_JIT_BUILD
 __global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ SweepParams P)
 {
     const uint32_t lane = threadIdx.x & 31u;
@@ -659,5 +660,6 @@ __global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ Sweep
     rec[32] = make_uint4(dlt.lo, dlt.hi, dund.lo, dund.hi);
     rec[64] = make_uint4(plt.lo, plt.hi, pund.lo, pund.hi);
 }
+#endif
 
 }  // namespace pcpd
