@@ -300,9 +300,9 @@ def ours_arm(args, cfg: wl.Config) -> None:
     e2e_steps = max(2, min(args.steps, 5))
 
     def e2e_step():
-        h.set_lattice_ptr(host_lat.data_ptr())       # H2D of the step's input lattice
-        h.run(SWEEPS_PER_STEP)
-        h.density_ptr(host_cnt.data_ptr())            # D2H of the step's result
+        # one call of the C ABI: H2D of the step's input lattice (cut into column chunks whose copies overlap the
+        # sweeps of the chunks before), SWEEPS_PER_STEP sweeps, density, D2H of the counts
+        h.step_from_host_ptr(host_lat.data_ptr(), SWEEPS_PER_STEP, host_cnt.data_ptr())
 
     e2e_step()
     barrier()
@@ -371,7 +371,8 @@ def ours_arm(args, cfg: wl.Config) -> None:
                     cpu_baseline=dict(value=cpu_rate, unit=UNIT, cores=cores, kind="oracle", sample=sample,
                                       lazy_blocks_per_attempt_word=LAST_ORACLE_LAZY_BLOCKS),
                     e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=cfg.lattice_bytes,
-                             d2h_bytes_per_step=4 * cfg.n_replicas, steps=e2e_steps, wall_s=wall),
+                             d2h_bytes_per_step=4 * cfg.n_replicas, steps=e2e_steps, wall_s=wall,
+                             call="pcpd_step_from_host(host lattice, 10 sweeps, host counts)"),
                     gpu_launches=int(launches), clocks=clocks)
         print(json.dumps(line), flush=True)
     h.close()

@@ -147,6 +147,16 @@ PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
 PCPD_API int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words);
 PCPD_API int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words);
 
+/* One step from a HOST lattice, pipelined: the same result as
+ *     pcpd_set_lattice(h, in_words); pcpd_run(h, n_sweeps); pcpd_density(h, out_counts);
+ * (out_counts may be NULL: no density), but the upload is cut into chunks of 8 word columns - columns never
+ * interact, so a chunk can run all its n_sweeps sweeps as soon as it has arrived - and the host-to-device copy of
+ * chunk c+1 (a strided 2-D copy out of the canonical [i][w] layout, on a copy stream) overlaps the sweeps of chunk c.
+ * in_words: canonical words[i*W + w], L*W uint64, pinned host memory for the copies to be asynchronous.  Handles
+ * with fewer than 16 word columns, or whose 8-column chunks would not fill the GPU, run the plain sequence.
+ * Synchronises.  Errors as the three calls. */
+PCPD_API int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, uint32_t *out_counts);
+
 /* Schedule / precision constants in force for this handle (T_s after
  * clamping; K = 32 planes), so an independent implementation can be run with
  * the same ones.  Any out pointer may be NULL. */

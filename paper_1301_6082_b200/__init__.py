@@ -34,7 +34,7 @@ EXPORTS = (
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
-    "pcpd_jit_selftest", "pcpd_split_launch_count",
+    "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -118,6 +118,8 @@ def load_library() -> C.CDLL:
     L.pcpd_jit_launch_count.restype = C.c_uint64
     L.pcpd_jit_selftest.argtypes = [C.c_int, C.c_uint32, C.c_uint32, u64p]
     L.pcpd_jit_selftest.restype = C.c_int
+    L.pcpd_step_from_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+    L.pcpd_step_from_host.restype = C.c_int
     L.pcpd_split_launch_count.argtypes = [C.c_void_p]
     L.pcpd_split_launch_count.restype = C.c_uint64
     _lib = L
@@ -261,6 +263,10 @@ class Pcpd:
 
     def set_lattice_ptr(self, host_ptr: int):
         _check(self._lib, self._lib.pcpd_set_lattice(self._h, host_ptr))
+
+    def step_from_host_ptr(self, host_lattice_ptr: int, n_sweeps: int, host_counts_ptr: int = 0):
+        """set_lattice + run(n_sweeps) + density with the upload pipelined against the sweeps (pcpd_step_from_host)."""
+        _check(self._lib, self._lib.pcpd_step_from_host(self._h, host_lattice_ptr, int(n_sweeps), host_counts_ptr or None))
 
     def density_ptr(self, host_ptr: int):
         _check(self._lib, self._lib.pcpd_density(self._h, host_ptr))

@@ -444,6 +444,84 @@ int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words)
     return check_launch("permute kernel");
 }
 
+// Column chunk of the pipelined step: 8 word columns (64-byte rows of the canonical host layout) when the handle has
+// at least 16 columns and a chunk is large enough to fill the GPU; otherwise no pipelining.
+static uint32_t step_chunk_columns(const pcpd_t *h)
+{
+    const char *e = getenv("PCPD_STEP_CHUNK");   // tuning hook: columns per chunk (0 = no pipelining)
+    if (e) {
+        const long v = atol(e);
+        return v <= 0 || (uint64_t)v >= h->W ? (uint32_t)h->W : (uint32_t)v;
+    }
+    if (h->W < 16 || (h->L / h->Ts) * 8 < 148ull * 14) return (uint32_t)h->W;
+    return 8u;
+}
+
+int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, uint32_t *out_counts)
+{
+    if (!h || !in_words) return fail(PCPD_ERR_ARG, "null argument");
+    if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    const uint32_t cw = step_chunk_columns(h);
+    const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
+    if (cw >= W || h->thr || h->force_block) {   // no pipelining: the plain sequence
+        int rc = pcpd_set_lattice(h, in_words);
+        if (rc == PCPD_OK) rc = pcpd_run(h, n_sweeps);
+        if (rc == PCPD_OK && out_counts) rc = pcpd_density(h, out_counts);
+        return rc;
+    }
+    const size_t bytes = 8 * h->L * h->W;
+    uint64_t *stage = (uint64_t *)dev_alloc(bytes, h->stream);
+    if (!stage) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
+    cudaStream_t copy = nullptr;
+    cudaError_t e = cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking);
+    const uint32_t nchunks = (W + cw - 1) / cw;
+    cudaEvent_t *ev = new (std::nothrow) cudaEvent_t[nchunks]();
+    cudaEvent_t start = nullptr;
+    if (e == cudaSuccess && !ev) e = cudaErrorMemoryAllocation;
+    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) e = cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming);
+    // the copies start once everything already queued on the handle's stream has finished with the lattice
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventRecord(start, h->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, start, 0);
+    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
+        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        uint64_t *dst = stage + (size_t)w0 * L;   // chunk held densely as [L][nw]
+        e = cudaMemcpy2DAsync(dst, (size_t)nw * 8, in_words + w0, (size_t)W * 8, (size_t)nw * 8, L, cudaMemcpyHostToDevice, copy);
+        if (e == cudaSuccess) e = cudaEventRecord(ev[c], copy);
+    }
+    int rc = PCPD_OK;
+    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
+        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        e = cudaStreamWaitEvent(h->stream, ev[c], 0);
+        if (e != cudaSuccess) break;
+        g_launches += launch_permute(stage + (size_t)w0 * L, h->lat + (size_t)w0 * L, L, nw, 1, 1, h->stream);
+        SweepParams Pc = h->P;   // the chunk as a lattice of its own: columns w0 .. w0+nw-1 (columns never interact)
+        Pc.lat = h->lat + (size_t)w0 * L;
+        Pc.W = nw;
+        Pc.word_offset = h->P.word_offset + w0;
+        for (uint64_t it = 0; it < n_sweeps; ++it) {
+            Pc.t = (uint32_t)(h->sweep + it);
+            g_launches += launch_sweep(Pc, h->variant, false, h->stream, &h->jit, nullptr);
+        }
+    }
+    if (e == cudaSuccess) {
+        h->sweep += n_sweeps;
+        rc = check_launch("pipelined step");
+        if (rc == PCPD_OK && out_counts) rc = pcpd_density(h, out_counts);
+        else if (rc == PCPD_OK) e = cudaStreamSynchronize(h->stream);
+    }
+    cudaStreamSynchronize(copy);
+    cudaStreamSynchronize(h->stream);
+    for (uint32_t c = 0; ev && c < nchunks; ++c)
+        if (ev[c]) cudaEventDestroy(ev[c]);
+    delete[] ev;
+    if (start) cudaEventDestroy(start);
+    if (copy) cudaStreamDestroy(copy);
+    dev_free(stage);
+    if (e != cudaSuccess) return cuda_fail(e, "step_from_host");
+    return rc;
+}
+
 int pcpd_schedule_info(const pcpd_t *h, uint32_t *Ts, uint32_t *D, uint32_t *A, uint32_t *K)
 {
     if (!h) return fail(PCPD_ERR_ARG, "null handle");

@@ -258,6 +258,40 @@ def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
         assert np.array_equal(x, y)
 
 
+def test_pipelined_step_from_host_equals_the_plain_sequence(pk, monkeypatch):
+    """pcpd_step_from_host (upload cut into column chunks, copy of chunk c+1 overlapping the sweeps of chunk c) must
+    give exactly what set_lattice + run + density give: forced 4-column chunks with a ragged last chunk at a small
+    size (also against the oracle), and the default 8-column chunks at cfg5's size."""
+    monkeypatch.setenv("PCPD_STEP_CHUNK", "4")
+    L, R = 4096, 64 * 6
+    w0 = wl.random_lattice_words(L, R // 64, 0.5, seed=3)
+    a = pk.Pcpd(L, R, 0.3, 0.12, 21, 0)
+    b = pk.Pcpd(L, R, 0.3, 0.12, 21, 0)
+    a.set_lattice(w0); a.sweep = 5; a.run(3)
+    b.sweep = 5
+    cnt = np.empty(R, dtype=np.uint32)
+    b.step_from_host_ptr(w0.ctypes.data, 3, cnt.ctypes.data)
+    assert b.sweep == 8
+    assert np.array_equal(a.get_lattice(), b.get_lattice()) and np.array_equal(a.density(), cnt)
+    o = oracle.Oracle(L, R, 0.3, 0.12, 21, 0)
+    o.set_words(w0); o.sweep = 5; o.run(3)
+    assert np.array_equal(b.get_lattice(), o.get_words()) and np.array_equal(cnt, o.counts())
+    a.close(); b.close()
+    monkeypatch.delenv("PCPD_STEP_CHUNK")
+    c = wl.BY_NAME["cfg5"]
+    import torch
+    host = torch.empty((c.L, c.W), dtype=torch.int64).pin_memory()
+    hn = host.numpy().view(np.uint64)
+    hn[:] = wl.random_lattice_words(c.L, c.W, 0.6, seed=4)
+    a = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
+    b = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
+    a.set_lattice_ptr(host.data_ptr()); a.run(2)
+    cnt = np.empty(c.n_replicas, dtype=np.uint32)
+    b.step_from_host_ptr(host.data_ptr(), 2, cnt.ctypes.data)
+    assert np.array_equal(a.get_lattice(), b.get_lattice()) and np.array_equal(a.density(), cnt)
+    a.close(); b.close()
+
+
 def test_word_offset_shards_equal_one_big_run(pk):
     kw = dict(d=0.3, p=0.12, seed=31, variant=0)
     big = pk.Pcpd(2048, 512, **kw)
