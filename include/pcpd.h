@@ -143,6 +143,15 @@ PCPD_API int pcpd_density(pcpd_t *h, uint32_t *out_counts);
  * replica r (pair density of PAPER.md:203-208, Figs 5-6).  Synchronises. */
 PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
 
+/* A whole time series in one call (the paper's observable is rho(t) at many times, Fig. 1; pair
+ * density PAPER.md:203-208): for k = 0 .. n_times-1 advance to sweep times[k] (absolute sweep indices, ascending,
+ * times[0] >= the current counter; equal entries allowed) and record the per-replica particle counts into
+ * out_counts[k*n_replicas + r] and / or the pair counts into out_pairs[k*n_replicas + r] (either may be NULL, not
+ * both).  Same numbers as pcpd_run + pcpd_density / pcpd_pair_density called in a loop, but the records stay on the
+ * device until the end: one read-back and one synchronisation for the series instead of one per record.
+ * PCPD_ERR_ARG for non-ascending times, PCPD_ERR_RANGE past 2^32 - 1; on error the counter stays where it got to. */
+PCPD_API int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs);
+
 /* Lattice in canonical order words[i*W + w], L*W uint64.  Synchronise. */
 PCPD_API int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words);
 PCPD_API int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words);

@@ -34,7 +34,7 @@ EXPORTS = (
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
-    "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host",
+    "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host", "pcpd_run_series",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -118,6 +118,8 @@ def load_library() -> C.CDLL:
     L.pcpd_jit_launch_count.restype = C.c_uint64
     L.pcpd_jit_selftest.argtypes = [C.c_int, C.c_uint32, C.c_uint32, u64p]
     L.pcpd_jit_selftest.restype = C.c_int
+    L.pcpd_run_series.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
+    L.pcpd_run_series.restype = C.c_int
     L.pcpd_step_from_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     L.pcpd_step_from_host.restype = C.c_int
     L.pcpd_split_launch_count.argtypes = [C.c_void_p]
@@ -241,6 +243,17 @@ class Pcpd:
         out = np.empty(self.n_replicas, dtype=np.uint32) if out is None else out
         _check(self._lib, self._lib.pcpd_density(self._h, out.ctypes.data))
         return out
+
+    def run_series(self, times, pairs=False):
+        """Advance to each of the ascending absolute sweep indices `times` and record the per-replica counts there
+        (pcpd_run_series: one read-back for the whole series).  Returns counts[len(times), n_replicas], and the pair
+        counts as well if pairs is true."""
+        t = np.ascontiguousarray(times, dtype=np.uint64)
+        cnt = np.empty((len(t), self.n_replicas), dtype=np.uint32)
+        pr = np.empty((len(t), self.n_replicas), dtype=np.uint32) if pairs else None
+        _check(self._lib, self._lib.pcpd_run_series(self._h, t.ctypes.data, len(t), cnt.ctypes.data,
+                                                    pr.ctypes.data if pairs else None))
+        return (cnt, pr) if pairs else cnt
 
     def pair_density(self, out=None) -> np.ndarray:
         out = np.empty(self.n_replicas, dtype=np.uint32) if out is None else out

@@ -404,6 +404,46 @@ static int density_impl(pcpd_t *h, uint32_t *out, int pairs)
 int pcpd_density(pcpd_t *h, uint32_t *out_counts) { return density_impl(h, out_counts, 0); }
 int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs) { return density_impl(h, out_pairs, 1); }
 
+int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs)
+{
+    if (!h || !times || n_times == 0 || (!out_counts && !out_pairs)) return fail(PCPD_ERR_ARG, "run_series: null argument");
+    for (uint64_t k = 0; k < n_times; ++k) {
+        if (times[k] < (k ? times[k - 1] : h->sweep)) return fail(PCPD_ERR_ARG, "run_series: times must ascend from the current sweep");
+        if (times[k] > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    }
+    const int nobs = (out_counts ? 1 : 0) + (out_pairs ? 1 : 0);
+    const size_t row = 4 * h->R, bytes = row * n_times * nobs;
+    uint32_t *series = (uint32_t *)dev_alloc(bytes, h->stream);
+    if (!series) return fail(PCPD_ERR_ALLOC, "run_series: allocation of %llu bytes failed", (unsigned long long)bytes);
+    cudaError_t e = cudaMemsetAsync(series, 0, bytes, h->stream);
+    int rc = PCPD_OK;
+    for (uint64_t k = 0; e == cudaSuccess && rc == PCPD_OK && k < n_times; ++k) {
+        rc = pcpd_run(h, times[k] - h->sweep);
+        if (rc != PCPD_OK) break;
+        uint32_t *dst = series + (size_t)k * h->R * nobs;   // record k: [counts][pairs]
+        if (out_counts) g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 0, dst, h->stream);
+        if (out_pairs)
+            g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 1, dst + (out_counts ? h->R : 0), h->stream);
+        rc = check_launch("density kernel");
+    }
+    // ONE read-back and ONE synchronisation for the whole series
+    if (e == cudaSuccess && rc == PCPD_OK) {
+        if (nobs == 1) {
+            e = cudaMemcpyAsync(out_counts ? out_counts : out_pairs, series, bytes, cudaMemcpyDeviceToHost, h->stream);
+        } else {
+            e = cudaMemcpy2DAsync(out_counts, row, series, 2 * row, row, n_times, cudaMemcpyDeviceToHost, h->stream);
+            if (e == cudaSuccess)
+                e = cudaMemcpy2DAsync(out_pairs, row, series + h->R, 2 * row, row, n_times, cudaMemcpyDeviceToHost, h->stream);
+        }
+    }
+    const cudaError_t es = cudaStreamSynchronize(h->stream);
+    dev_free(series);
+    if (rc != PCPD_OK) return rc;
+    if (e == cudaSuccess) e = es;
+    if (e != cudaSuccess) return cuda_fail(e, "run_series");
+    return PCPD_OK;
+}
+
 int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words)
 {
     if (!h || !out_words) return fail(PCPD_ERR_ARG, "null argument");

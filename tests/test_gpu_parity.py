@@ -292,6 +292,30 @@ def test_pipelined_step_from_host_equals_the_plain_sequence(pk, monkeypatch):
     a.close(); b.close()
 
 
+def test_run_series_equals_run_and_density_in_a_loop(pk):
+    """pcpd_run_series (records kept on the device, one read-back) against the oracle's counts at the same times and
+    against pcpd_run + pcpd_density / pcpd_pair_density in a loop; argument errors."""
+    L, R = 4096, 128
+    times = [0, 1, 2, 2, 5, 9]
+    a = pk.Pcpd(L, R, 0.3, 0.12, 31, 0)
+    b = pk.Pcpd(L, R, 0.3, 0.12, 31, 0)
+    o = oracle.Oracle(L, R, 0.3, 0.12, 31, 0)
+    a.init(1); b.init(1); o.init(1)
+    cnt, pr = a.run_series(times, pairs=True)
+    assert a.sweep == 9
+    for k, t in enumerate(times):
+        b.run(t - b.sweep)
+        o.run(t - o.sweep)
+        assert np.array_equal(cnt[k], b.density()) and np.array_equal(pr[k], b.pair_density())
+        assert np.array_equal(cnt[k], o.counts()) and np.array_equal(pr[k], o.pair_counts())
+    assert np.array_equal(a.run_series([9, 12]), np.stack([b.density(), (b.run(3), b.density())[1]]))
+    with pytest.raises(pk.PcpdError):
+        a.run_series([11])          # behind the counter
+    with pytest.raises(pk.PcpdError):
+        a.run_series([13, 12])      # not ascending
+    a.close(); b.close()
+
+
 def test_word_offset_shards_equal_one_big_run(pk):
     kw = dict(d=0.3, p=0.12, seed=31, variant=0)
     big = pk.Pcpd(2048, 512, **kw)
