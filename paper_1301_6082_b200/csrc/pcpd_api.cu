@@ -210,6 +210,7 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         h->jit.mode = !jm ? 1 : !strcmp(jm, "0") ? 0 : !strcmp(jm, "force") ? 2 : 1;
         h->jit.state = 0;
         h->jit.kernel = nullptr;
+        h->jit.wpb = 0;
     }
     memset(&h->split, 0, sizeof h->split);
     h->stream = nullptr;

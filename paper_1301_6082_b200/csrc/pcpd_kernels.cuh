@@ -55,6 +55,7 @@ struct JitSlot {
     int mode;      // 0 off, 1 auto (large problems only), 2 always (test hook)
     int state;     // 0 not tried yet, 1 kernel ready, -1 unavailable (the built-in kernel is used)
     void *kernel;  // CUfunction
+    int wpb;       // warps per block the kernel was compiled for (launches with another shape use the built-in kernel)
 };
 
 // SPLIT path of one handle (small problems).  The masks of a sweep depend on (seed, t, schedule, thresholds) only, not

@@ -204,8 +204,9 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
             js.Td = P.thd.T32; js.Tp = P.thp.T32; js.Ts = P.Ts; js.D = P.D; js.A = P.A; js.L = P.L;
             jit->kernel = jit_sweep_kernel(js, wpb >= 4 ? 116 * 1024 : 226 * 1024);
             jit->state = jit->kernel ? 1 : -1;
+            jit->wpb = wpb;
         }
-        if (jit->state == 1) {
+        if (jit->state == 1 && jit->wpb == wpb) {
             const uint32_t ntasks = (P.L / P.Ts) * P.W;
             if (jit_launch(jit->kernel, P, (ntasks + wpb - 1) / wpb, wpb * 32, warp_smem_bytes(P.Ts, wpb), stream) == 0)
                 return 1;

@@ -270,6 +270,23 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
     und = Mask2{ulo, uhi};
 }
 
+// Threshold-specialised compare of ONE more block M (planes 2M, 2M+1) on top of an exact (lt, und): the lanes still
+// equal to T that fall below T's two bits join lt, those that match them stay undecided.  3 LOP3 per 32-lane half.
+template <uint32_t T, int M>
+__device__ __forceinline__ void tail_spec(Mask2 &lt, Mask2 &und, const U4 &b)
+{
+    constexpr bool t0 = (T >> (31 - 2 * M)) & 1u, t1 = 2 * M + 1 < 32 ? (T >> (30 - 2 * M)) & 1u : 0u;
+    const uint32_t p0[2] = {b.x0, b.x1}, p1[2] = {b.x2, b.x3};
+    uint32_t *l[2] = {&lt.lo, &lt.hi}, *u[2] = {&und.lo, &und.hi};
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const uint32_t e0 = t0 ? p0[h] : ~p0[h], e1 = t1 ? p1[h] : ~p1[h];          // plane bit equals T's bit
+        const uint32_t less = (t0 ? ~p0[h] : 0u) | (e0 & (t1 ? ~p1[h] : 0u));       // two-bit value below T's two bits
+        *l[h] |= *u[h] & less;
+        *u[h] &= e0 & e1;
+    }
+}
+
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
@@ -495,6 +512,16 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t m = nud;
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
+                if constexpr (SPEC && NU_D < (int)nblk_of(STD)) {
+                    // first tail block with T's bits as constants (most tail work is this iteration)
+                    if (__any_sync(0xffffffffu, (dund.lo | dund.hi) != 0)) {
+                        tail_spec<STD, NU_D>(dlt, dund, philox_block(STREAM_DIFF | NU_D, ps, pw, rk));
+                        ++m;
+                        Tsh <<= 2;
+                    } else {
+                        m = nblkD;   // nothing undecided: skip the loop's vote as well
+                    }
+                }
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
                     if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
@@ -524,6 +551,15 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t Tsh = Tp << (2 * nup);
                 uint32_t m = nup;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
+                if constexpr (SPEC && NU_P < (int)nblk_of(STP)) {
+                    if (__any_sync(0xffffffffu, (pund.lo | pund.hi) != 0)) {
+                        tail_spec<STP, NU_P>(plt, pund, philox_block(STREAM_ANNI | NU_P, ps, pw, rk));
+                        ++m;
+                        Tsh <<= 2;
+                    } else {
+                        m = nblkP;
+                    }
+                }
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
                     if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
