@@ -116,7 +116,10 @@ size_t split_mask_bytes(const SweepParams &P) { return (size_t)(P.L / P.Ts) * P.
 // Small problems (SplitSlot::buf allocated by the API layer when the handle qualifies): two launches per sweep.
 int split_setup(SplitSlot *s)
 {
-    if (cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking) != cudaSuccess) return -1;
+    // lowest priority: mask_kernel's many blocks must not delay the update kernel's, which are the critical path
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if (cudaStreamCreateWithPriority(&s->aux, cudaStreamNonBlocking, prio_lo) != cudaSuccess) return -1;
     for (int i = 0; i < 2; ++i) {
         if (cudaEventCreateWithFlags(&s->ready[i], cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&s->freed[i], cudaEventDisableTiming) != cudaSuccess)

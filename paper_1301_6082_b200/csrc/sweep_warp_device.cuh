@@ -270,23 +270,6 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
     und = Mask2{ulo, uhi};
 }
 
-// Threshold-specialised compare of ONE more block M (planes 2M, 2M+1) on top of an exact (lt, und): the lanes still
-// equal to T that fall below T's two bits join lt, those that match them stay undecided.  3 LOP3 per 32-lane half.
-template <uint32_t T, int M>
-__device__ __forceinline__ void tail_spec(Mask2 &lt, Mask2 &und, const U4 &b)
-{
-    constexpr bool t0 = (T >> (31 - 2 * M)) & 1u, t1 = 2 * M + 1 < 32 ? (T >> (30 - 2 * M)) & 1u : 0u;
-    const uint32_t p0[2] = {b.x0, b.x1}, p1[2] = {b.x2, b.x3};
-    uint32_t *l[2] = {&lt.lo, &lt.hi}, *u[2] = {&und.lo, &und.hi};
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        const uint32_t e0 = t0 ? p0[h] : ~p0[h], e1 = t1 ? p1[h] : ~p1[h];          // plane bit equals T's bit
-        const uint32_t less = (t0 ? ~p0[h] : 0u) | (e0 & (t1 ? ~p1[h] : 0u));       // two-bit value below T's two bits
-        *l[h] |= *u[h] & less;
-        *u[h] &= e0 & e1;
-    }
-}
-
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
@@ -315,7 +298,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     // arithmetic, seam bookkeeping and the mulhi by n_allow then work on immediates).
     const uint32_t Ts = SPEC ? CTS : P.Ts, D = SPEC ? CD : P.D, A = SPEC ? CA : P.A, L = SPEC ? CL : P.L;
     const uint32_t S = SPEC ? CD / (CA ? CA : 1u) : P.S, n = SPEC ? CTS / (CD ? CD : 1u) : P.n, t = P.t;
-    const RoundKeys &rk = P.rk;  // (baking the seed in as well was measured slower: 32-bit immediates in the xor chain)
+    // (baking the seed in as well was measured slower: 32-bit immediates in the xor chain)
+    const RoundKeys &rk = P.rk;
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     const uint32_t ntiles = L / Ts;
@@ -341,6 +325,29 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
     const uint32_t odd = vec ? (start & 1u) : 0u;
     uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
+    // SPLIT consumer (WPB = 1): the records of this task's J = S*A attempts (three rows of 32 uint4 each, contiguous
+    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies, one per sub-step (A
+    // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
+    // records when it gets there, and reads each record one attempt ahead of its use.
+    const uint32_t nud = SPLIT == 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT == 2 ? P.split_nup : (uint32_t)NU_P;
+    const uint4 *mrec = nullptr;
+    uint64_t *bars = nullptr;
+    uint4 nx0{}, nx1{}, nx2{};
+    if constexpr (SPLIT == 2) {
+        const uint32_t J = S * A, cbytes = A * MASK_REC_BYTES;
+        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
+        bars = reinterpret_cast<uint64_t *>(mbase + (size_t)J * MASK_REC_BYTES);
+        if (lane == 0) {
+            for (uint32_t c = 0; c < S; ++c) mbar_init(bars + c, 1u);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            const uint8_t *src = reinterpret_cast<const uint8_t *>(P.mask_dev) + (size_t)task * J * MASK_REC_BYTES;
+            for (uint32_t c = 0; c < S; ++c) {
+                mbar_expect_tx(bars + c, cbytes);
+                bulk_g2s(mbase + (size_t)c * cbytes, src + (size_t)c * cbytes, cbytes, bars + c);
+            }
+        }
+        mrec = reinterpret_cast<const uint4 *>(mbase) + lane;   // (issued before the tile load so that the two overlap)
+    }
     if (vec) {
         const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
         const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
@@ -405,30 +412,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 
-    // SPLIT consumer (WPB = 1): the records of this task's J = S*A attempts (three rows of 32 uint4 each, contiguous
-    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies, one per sub-step (A
-    // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
-    // records when it gets there, and reads each record one attempt ahead of its use.
-    const uint32_t nud = SPLIT == 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT == 2 ? P.split_nup : (uint32_t)NU_P;
-    const uint4 *mrec = nullptr;
-    uint64_t *bars = nullptr;
-    uint4 nx0{}, nx1{}, nx2{};
-    if constexpr (SPLIT == 2) {
-        const uint32_t J = S * A, cbytes = A * MASK_REC_BYTES;
-        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
-        bars = reinterpret_cast<uint64_t *>(mbase + (size_t)J * MASK_REC_BYTES);
-        if (lane == 0) {
-            for (uint32_t c = 0; c < S; ++c) mbar_init(bars + c, 1u);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            const uint8_t *src = reinterpret_cast<const uint8_t *>(P.mask_dev) + (size_t)task * J * MASK_REC_BYTES;
-            for (uint32_t c = 0; c < S; ++c) {
-                mbar_expect_tx(bars + c, cbytes);
-                bulk_g2s(mbase + (size_t)c * cbytes, src + (size_t)c * cbytes, cbytes, bars + c);
-            }
-        }
-        __syncwarp();
-        mrec = reinterpret_cast<const uint4 *>(mbase) + lane;
-    }
 #pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
         DomainPos dp{};
@@ -512,16 +495,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t m = nud;
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
-                if constexpr (SPEC && NU_D < (int)nblk_of(STD)) {
-                    // first tail block with T's bits as constants (most tail work is this iteration)
-                    if (__any_sync(0xffffffffu, (dund.lo | dund.hi) != 0)) {
-                        tail_spec<STD, NU_D>(dlt, dund, philox_block(STREAM_DIFF | NU_D, ps, pw, rk));
-                        ++m;
-                        Tsh <<= 2;
-                    } else {
-                        m = nblkD;   // nothing undecided: skip the loop's vote as well
-                    }
-                }
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
                     if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
@@ -551,15 +524,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t Tsh = Tp << (2 * nup);
                 uint32_t m = nup;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
-                if constexpr (SPEC && NU_P < (int)nblk_of(STP)) {
-                    if (__any_sync(0xffffffffu, (pund.lo | pund.hi) != 0)) {
-                        tail_spec<STP, NU_P>(plt, pund, philox_block(STREAM_ANNI | NU_P, ps, pw, rk));
-                        ++m;
-                        Tsh <<= 2;
-                    } else {
-                        m = nblkP;
-                    }
-                }
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
                     if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
