@@ -196,12 +196,12 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
     // kernel below computes the same thing.
     if (jit && jit->mode && jit->state >= 0 && (jit->mode == 2 || wpb == 7) && !P.thd.all && !P.thp.all) {
         if (jit->state == 0) {
-            // prefix lengths of the specialised kernel: all of a short threshold's blocks, else 6 DIFF / 4 ANNI
-            // (tuned on B200 at cfg3-5: its prefix compare is cheaper than the built-in kernel's, so 6 beats 5)
+            // prefix lengths of the specialised kernel: all of a short threshold's blocks, else 6 DIFF / 4 ANNI (5 for
+            // TCPD and QCPD) (tuned on B200 at cfg3-5: its prefix compare is cheaper than the built-in kernel's)
             JitSpec js;
             js.variant = variant; js.wpb = wpb; js.pmode = P.pmask_paper ? 1 : 0;
             js.nud = (int)min((P.thd.nplanes + 1) >> 1, 6u);
-            js.nup = P.pmask_paper ? 1 : (int)min((P.thp.nplanes + 1) >> 1, 4u);
+            js.nup = P.pmask_paper ? 1 : (int)min((P.thp.nplanes + 1) >> 1, variant == 1 || variant == 2 ? 5u : 4u);
             if (const char *e = getenv("PCPD_JIT_NUD")) js.nud = atoi(e);   // tuning hooks
             if (const char *e = getenv("PCPD_JIT_NUP")) js.nup = atoi(e);
             js.Td = P.thd.T32; js.Tp = P.thp.T32; js.Ts = P.Ts; js.D = P.D; js.A = P.A; js.L = P.L;
