@@ -210,8 +210,12 @@ PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t
  * ALL attempts of the sweep in parallel (MISC block, compared prefix planes of DIFF and ANNI), then the update
  * kernel reads them and applies the attempts in order; the masks do not depend on the lattice, so those of
  * sweep t+1 are computed on an internal auxiliary stream while sweep t is applied.  Same results bit for bit.  Environment, read by
- * pcpd_create*: PCPD_SPLIT=0 never; PCPD_SPLIT=force whenever the mask buffer stays below 1 GiB (test hook).
- * pcpd_split_launch_count: kernels this handle has launched on that path (2 per sweep + 1; 0 = fused kernel). */
+ * Handles with more tile columns than SMs but at most 512 use a one-kernel form of the same idea: one block of
+ * four warps per tile column, three producer warps computing the records into a shared-memory ring, one update warp.
+ * pcpd_create*: PCPD_SPLIT=0 never; PCPD_SPLIT=force the two-kernel path whenever the mask buffer stays below
+ * 1 GiB, PCPD_SPLIT=block the one-block form at every size (test hooks).
+ * pcpd_split_launch_count: kernels this handle has launched on those paths (two-kernel: 2 per sweep + 1; one-block
+ * form: 1 per sweep; 0 = fused kernel). */
 PCPD_API uint64_t pcpd_split_launch_count(const pcpd_t *h);
 
 /* Number of kernels this library has launched so far in this process. */

@@ -255,10 +255,17 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         // B200 at L = 65536: 128 columns 75 -> 38 us per sweep, 256 columns 76 -> 70 us, 512 columns 76 -> 140 us);
         // "0" never; "force" whenever the mask buffer stays below 1 GiB.
         const char *sm = getenv("PCPD_SPLIT");
-        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : 1;
+        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : !strcmp(sm, "block") ? 3 : 1;
+        // more than one tile column per SM but still too few to fill the GPU (measured on B200 up to 512: 256 columns
+        // 76 -> 47 us per sweep, 512 columns 76 -> 69 us): producer warps and the update warp in one block per tile
+        // column, records through a shared-memory ring ("block": that path at every size - test hook)
+        const uint64_t ntasks0 = (L / Ts) * W;
+        if ((mode == 3 || (mode == 1 && ntasks0 > (uint64_t)prop.multiProcessorCount && ntasks0 <= 512)) &&
+            split_block_supported(Ts, D) && !h->force_block)
+            h->split.block_mode = 1;
         const uint64_t ntasks = (L / Ts) * W;
         const size_t bytes = split_mask_bytes(P);
-        if (mode && split_supported(Ts, D) && !h->force_block &&
+        if (mode && mode != 3 && split_supported(Ts, D) && !h->force_block &&
             (mode == 2 ? bytes <= (1ull << 30) : ntasks <= (uint64_t)prop.multiProcessorCount)) {
             h->split.buf[0] = dev_alloc(bytes, h->stream);   // any failure here: the fused kernel is used
             h->split.buf[1] = h->split.buf[0] ? dev_alloc(bytes, h->stream) : nullptr;
@@ -332,6 +339,7 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
     }
     h->P.thr_dev = h->thr;
     h->force_block = false;
+    h->split.block_mode = 0;
     split_teardown(&h->split);   // per-word thresholds run the fused kernel
     dev_free(h->split.buf[0]);
     dev_free(h->split.buf[1]);

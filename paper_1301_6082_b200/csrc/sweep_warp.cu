@@ -111,6 +111,51 @@ static int split_consumer_any(int variant, int pmode, const SweepParams *P, cuda
     }
 }
 
+// ---- SPLIT = 3: producer warps and the update warp in ONE block per tile column (records through a shared-memory ring)
+static size_t block4_smem_bytes(uint32_t Ts)
+{
+    return ((warp_smem_bytes(Ts, 1) + 127) & ~(size_t)127) + (size_t)RING_SLOTS * MASK_REC_BYTES + 2 * RING_SLOTS * 8;
+}
+
+bool split_block_supported(uint32_t Ts, uint32_t D) { return sweep_warp_supported(Ts, D) && block4_smem_bytes(Ts) <= 226 * 1024; }
+
+template <int VARIANT, int PMODE>
+static int block4_op(const SweepParams *P, cudaStream_t stream)
+{
+    auto kern = sweep_warp_kernel<VARIANT, 4, 0, 0, PMODE, 0, 0, 0u, 0u, 0u, 0u, 0u, 0u, 3>;
+    if (!P) return (int)cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+    kern<<<(P->L / P->Ts) * P->W, 128, block4_smem_bytes(P->Ts), stream>>>(*P);
+    return 1;
+}
+
+static int block4_any(int variant, int pmode, const SweepParams *P, cudaStream_t stream)
+{
+    switch (variant * 2 + pmode) {
+    case 0: return block4_op<0, 0>(P, stream);
+    case 1: return block4_op<0, 1>(P, stream);
+    case 2: return block4_op<1, 0>(P, stream);
+    case 3: return block4_op<1, 1>(P, stream);
+    case 4: return block4_op<2, 0>(P, stream);
+    case 5: return block4_op<2, 1>(P, stream);
+    case 6: return block4_op<3, 0>(P, stream);
+    default: return block4_op<3, 1>(P, stream);
+    }
+}
+
+static int launch_sweep_block4(const SweepParams &P0, int variant, cudaStream_t stream, SplitSlot *split)
+{
+    SweepParams P = P0;
+    uint32_t cap_d = 7u, cap_p = 5u;   // tuned on B200 (L = 65536, 256 .. 512 tile columns); the producers are issue-bound
+    if (const char *e = getenv("PCPD_SPLIT_NUD")) cap_d = (uint32_t)atoi(e);   // tuning hooks
+    if (const char *e = getenv("PCPD_SPLIT_NUP")) cap_p = (uint32_t)atoi(e);
+    P.split_nud = min((P.thd.nplanes + 1u) >> 1, cap_d);
+    P.split_nup = P.pmask_paper ? 1u : min((P.thp.nplanes + 1u) >> 1, cap_p);
+    P.rr = variant == 3 ? 1u : 2u + (uint32_t)variant;
+    block4_any(variant, P.pmask_paper ? 1 : 0, &P, stream);
+    split->launches += 1;
+    return 1;
+}
+
 size_t split_mask_bytes(const SweepParams &P) { return (size_t)(P.L / P.Ts) * P.W * P.S * P.A * 96u * sizeof(uint4); }
 
 // Small problems (SplitSlot::buf allocated by the API layer when the handle qualifies): two launches per sweep.
@@ -188,6 +233,7 @@ static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t s
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split)
 {
     if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
+    if (split && split->block_mode && !(jit && jit->mode == 2)) return launch_sweep_block4(P, variant, stream, split);
     if (split && split->buf[0] && !(jit && jit->mode == 2)) return launch_sweep_split(P, variant, stream, split);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
     const int nud = nu_d_of((P.thd.nplanes + 1) >> 1);
@@ -234,7 +280,8 @@ int configure_warp_kernels()
         }
     for (int variant = 0; variant < 4; ++variant)
         for (int pmode = 0; pmode < 2; ++pmode) {
-            const int e = split_consumer_any(variant, pmode, nullptr, nullptr);
+            int e = split_consumer_any(variant, pmode, nullptr, nullptr);
+            if (e == 0) e = block4_any(variant, pmode, nullptr, nullptr);
             if (e != 0) return e;
         }
     return 0;

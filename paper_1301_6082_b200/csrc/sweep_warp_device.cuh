@@ -270,6 +270,70 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
     und = Mask2{ulo, uhi};
 }
 
+// Everything of attempt j of tile column `task` that does not depend on the lattice (the producer side of the two
+// SPLIT paths): the MISC block (fission-side mask, and the footprint position resolved to the tile-local index of
+// site x-1 with the sub-step's inner shift and seam), and the generic-threshold compare of the first P.split_nud
+// DIFF and P.split_nup ANNI blocks (the paper's gated mask when P.pmask_paper), written as three rows of 32 uint4:
+// rec[0] = {misc x0, x1, y0, x3}, rec[32] = {dlt, dund}, rec[64] = {plt, pund}  (rec already offset by the lane).
+__device__ __forceinline__ void produce_record(const SweepParams &P, uint32_t task, uint32_t j, uint32_t lane, uint32_t sigma,
+                                               uint4 *rec)
+{
+    const uint32_t ntiles = P.L / P.Ts;
+    const uint32_t tau = task % ntiles, wl = task / ntiles;
+    const uint32_t b = lane < P.n ? lane : 0u;
+    const RoundKeys &rk = P.rk;
+    const DomainPos dp = domain_pos(b, P.n, sigma, P.D, P.rr);
+    const PhiloxWarp pw = philox_warp_consts(P.t, P.word_offset + wl, rk);
+    const PhiloxSlot ps = philox_slot_consts((tau * P.n + b) * P.D + j, pw, rk);
+    Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
+    U4 misc, blk[4];
+    // blocks in groups of four independent chains (the prefix lengths are run-time values here)
+    {
+        const uint32_t c3s[4] = {STREAM_MISC, STREAM_DIFF | 0u, STREAM_DIFF | 1u, STREAM_DIFF | 2u};
+        philox_blocks<4>(c3s, ps, pw, rk, blk);
+        misc = blk[0];
+#pragma unroll
+        for (uint32_t i = 0; i < 3; ++i)
+            if (i < P.split_nud)
+                cmp_block_sum(dlt, dund, blk[1 + i], P.tdm[2 * i], P.tdm[2 * i + 1], P.sd[2 * i], P.sd[2 * i + 1]);
+    }
+    for (uint32_t m = 3; m < P.split_nud; m += 4) {
+        const uint32_t c3s[4] = {STREAM_DIFF | m, STREAM_DIFF | (m + 1u), STREAM_DIFF | (m + 2u), STREAM_DIFF | (m + 3u)};
+        philox_blocks<4>(c3s, ps, pw, rk, blk);
+#pragma unroll
+        for (uint32_t i = 0; i < 4; ++i)
+            if (m + i < P.split_nud)
+                cmp_block_sum(dlt, dund, blk[i], P.tdm[2 * (m + i)], P.tdm[2 * (m + i) + 1], P.sd[2 * (m + i)],
+                              P.sd[2 * (m + i) + 1]);
+    }
+    if (!P.pmask_paper) {
+        for (uint32_t m = 0; m < P.split_nup; m += 4) {
+            const uint32_t c3s[4] = {STREAM_ANNI | m, STREAM_ANNI | (m + 1u), STREAM_ANNI | (m + 2u), STREAM_ANNI | (m + 3u)};
+            philox_blocks<4>(c3s, ps, pw, rk, blk);
+#pragma unroll
+            for (uint32_t i = 0; i < 4; ++i)
+                if (m + i < P.split_nup)
+                    cmp_block_sum(plt, pund, blk[i], P.tpm[2 * (m + i)], P.tpm[2 * (m + i) + 1], P.sp[2 * (m + i)],
+                                  P.sp[2 * (m + i) + 1]);
+        }
+    } else {
+        const U4 pb = philox_block(STREAM_ANNI, ps, pw, rk);
+        const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
+        plt.lo = pb.x0 & pb.x2 & gate;
+        plt.hi = pb.x1 & pb.x3 & gate;
+    }
+    const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
+    rec[0] = make_uint4(misc.x0, misc.x1, y0, misc.x3);
+    rec[32] = make_uint4(dlt.lo, dlt.hi, dund.lo, dund.hi);
+    rec[64] = make_uint4(plt.lo, plt.hi, pund.lo, pund.hi);
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+constexpr uint32_t RING_SLOTS = 12u;   // SPLIT = 3: records in flight between the producer warps and the update warp
+
 }  // namespace
 
 // NU_D / NU_P = number of DIFF / ANNI blocks of an attempt evaluated unconditionally (template
@@ -303,8 +367,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     const uint32_t ntiles = L / Ts;
-    const uint32_t task = blockIdx.x * WPB + warp;
-    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel
+    const uint32_t task = SPLIT == 3 ? blockIdx.x : blockIdx.x * WPB + warp;
+    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel (but see SPLIT = 3)
 
     // C5 step 1: shifts from the SHIFT stream; lane j holds sigma_{k0+j} of the current group of 32 sub-steps.
     uint32_t sig_reg, Sigma;
@@ -320,7 +384,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     const uint32_t start = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts) % L);
     uint64_t *g = P.lat + (size_t)wl * L;             // column wl, contiguous in the site index
     const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
-    uint64_t *buf = smem + (size_t)warp * stride;
+    uint64_t *buf = smem + (SPLIT == 3 ? (size_t)0 : (size_t)warp * stride);
     const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
     const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
     const uint32_t odd = vec ? (start & 1u) : 0u;
@@ -329,7 +393,46 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies, one per sub-step (A
     // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
     // records when it gets there, and reads each record one attempt ahead of its use.
-    const uint32_t nud = SPLIT == 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT == 2 ? P.split_nup : (uint32_t)NU_P;
+    const uint32_t nud = SPLIT >= 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT >= 2 ? P.split_nup : (uint32_t)NU_P;
+    // SPLIT = 3 (WPB = 4, ONE tile column per block): warps 1-3 are producers - they compute the records of the
+    // column's attempts (produce_record), attempt j by warp 1 + j mod 3, into a ring of RING_SLOTS records in shared
+    // memory behind the tile - and warp 0 is the update warp.  Per slot a `full` mbarrier (the producer's lane 0
+    // arrives once its warp has written the record) and an `empty` one (the update warp's lane 0 arrives once its
+    // warp has read it); no global mask buffer, no second kernel.
+    uint4 *ring = nullptr;
+    uint64_t *fullb = nullptr, *emptyb = nullptr;
+    if constexpr (SPLIT == 3) {
+        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
+        ring = reinterpret_cast<uint4 *>(mbase);
+        fullb = reinterpret_cast<uint64_t *>(mbase + (size_t)RING_SLOTS * MASK_REC_BYTES);
+        emptyb = fullb + RING_SLOTS;
+        if (threadIdx.x == 0) {
+            for (uint32_t c = 0; c < RING_SLOTS; ++c) {
+                mbar_init(fullb + c, 1u);
+                mbar_init(emptyb + c, 1u);
+            }
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        if (warp != 0) {
+            const uint32_t J = S * A;
+            uint32_t sig = 0u, sig_group = ~0u;   // lane l holds sigma of sub-step 32 * sig_group + l
+            for (uint32_t j = warp - 1u; j < J; j += 3u) {
+                const uint32_t kk = j / A;
+                if ((kk >> 5) != sig_group) {
+                    sig_group = kk >> 5;
+                    sig = __umulhi(philox4x32_10(32u * sig_group + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
+                }
+                const uint32_t sigma = __shfl_sync(0xffffffffu, sig, kk & 31u);
+                const uint32_t slot = j % RING_SLOTS, pass = j / RING_SLOTS;
+                mbar_wait(emptyb + slot, (pass & 1u) ^ 1u);   // (a fresh barrier passes a wait on parity 1)
+                produce_record(P, task, j, lane, sigma, ring + slot * 96u + lane);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(fullb + slot);
+            }
+            return;
+        }
+    }
     const uint4 *mrec = nullptr;
     uint64_t *bars = nullptr;
     uint4 nx0{}, nx1{}, nx2{};
@@ -419,7 +522,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             mbar_wait(bars + k, 0u);
             nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64];
         }
-        if constexpr (SPLIT != 2) {  // (SPLIT consumer: mask_kernel has resolved the positions)
+        if constexpr (SPLIT < 2) {  // (SPLIT consumers: the producer has resolved the positions)
             if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
             const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
             dp = domain_pos(b, n, sigma, D, Rr);
@@ -431,10 +534,20 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
             // back to back so that the FMA pipe always has several wide multiplies in flight.
             PhiloxSlot ps{};
-            if constexpr (SPLIT != 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
+            if constexpr (SPLIT < 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
             U4 blks[1 + NU_D + NU_P];
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-            if constexpr (SPLIT == 2) {
+            if constexpr (SPLIT == 3) {
+                const uint32_t j = k * A + a, slot = j % RING_SLOTS, pass = j / RING_SLOTS;
+                mbar_wait(fullb + slot, pass & 1u);
+                const uint4 *r = ring + slot * 96u + lane;
+                const uint4 r0 = r[0], r1 = r[32], r2 = r[64];
+                __syncwarp();
+                if (lane == 0) mbar_arrive(emptyb + slot);
+                blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
+                dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
+                plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
+            } else if constexpr (SPLIT == 2) {
                 // this attempt's record was fetched during the previous attempt; fetch the next one of the sub-step now
                 const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
                 mrec += 96;
@@ -455,7 +568,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
 
             // C4: MISC block: Fm = ~lo (1 -> fission low, Alg. 1: r3 < 1/2), x2 -> position.
-            const uint32_t y0 = SPLIT == 2 ? misc.x2 : footprint_start(misc.x2, dp, Ts);  // (SPLIT: resolved by mask_kernel)
+            const uint32_t y0 = SPLIT >= 2 ? misc.x2 : footprint_start(misc.x2, dp, Ts);  // (SPLIT: resolved by the producer)
             const uint64_t Fm = ~lo64(misc);
             uint64_t *q = tile + y0;
             uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0, sg = 0;
@@ -469,8 +582,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
             // dependence on the state), the lazy tails only on the lanes whose outcome can matter:
             // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
-            if constexpr (SPLIT == 2) {
-                // prefix compared by mask_kernel
+            if constexpr (SPLIT >= 2) {
+                // prefix compared by the producer
             } else if constexpr (SPEC) {
                 prefix_spec<STD, NU_D>(dlt, dund, dblk);
                 if constexpr (PMODE == 0) prefix_spec<STP, NU_P>(plt, pund, pblk);
@@ -496,7 +609,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
-                    if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
+                    if constexpr (SPLIT >= 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -525,7 +638,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t m = nup;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
-                    if constexpr (SPLIT == 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
+                    if constexpr (SPLIT >= 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -544,7 +657,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
                 // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
                 // word-wide draw that is 1 w.p. 4p (x3 of the MISC block against floor(4p * 2^32)).
-                if constexpr (SPLIT != 2) {  // (SPLIT consumer: mask_kernel has done this)
+                if constexpr (SPLIT < 2) {  // (SPLIT consumers: the producer has done this)
                     const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
                     plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
                     plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
@@ -617,13 +730,10 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     }
 }
 
-// mask_kernel - producer of the SPLIT path: one warp per (tile column task, attempt j of the sweep); lane = domain.
-// Computes everything of an attempt that does not depend on the lattice: the MISC block (fission-side mask and the
-// footprint position, resolved to the tile-local index of site x-1 with the sub-step's inner shift and seam), and the
-// generic-threshold compare of the first P.split_nud DIFF and P.split_nup ANNI blocks (the paper's gated mask when
-// P.pmask_paper), and stores them as three coalesced uint4 rows per attempt: {misc x0, x1, y0, x3}, {dlt, dund},
-// {plt, pund}.  The blocks of a warp are evaluated one after the other (run-time loop): the parallelism is across the
-// (L / T_s) * W * D warps of the grid.  (Not part of the run-time specialised build, which is for large problems.)
+// mask_kernel - producer of the two-kernel SPLIT path: one warp per (tile column task, attempt j of the sweep), lane =
+// domain; stores the records (produce_record) coalesced into P.mask_dev.  The blocks of a warp are evaluated one after
+// the other (run-time loop): the parallelism is across the (L / T_s) * W * D warps of the grid.  (Not part of the
+// run-time specialised build, which is for large problems.)
 #ifndef PCPD_JIT_BUILD
 __global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ SweepParams P)
 {
@@ -632,33 +742,8 @@ __global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ Sweep
     const uint32_t gw = blockIdx.x * 4u + (threadIdx.x >> 5);
     if (gw >= ntiles * P.W * J) return;
     const uint32_t task = gw / J, j = gw - task * J;
-    const uint32_t tau = task % ntiles, wl = task / ntiles;
-    const uint32_t b = lane < P.n ? lane : 0u;
-    const RoundKeys &rk = P.rk;
-    const uint32_t sigma = __umulhi(philox4x32_10(j / P.A, P.t, 0u, STREAM_SHIFT, rk).x0, P.D);  // C5 step 1
-    const DomainPos dp = domain_pos(b, P.n, sigma, P.D, P.rr);
-    const PhiloxWarp pw = philox_warp_consts(P.t, P.word_offset + wl, rk);
-    const PhiloxSlot ps = philox_slot_consts((tau * P.n + b) * P.D + j, pw, rk);
-    const U4 misc = philox_block(STREAM_MISC, ps, pw, rk);
-    const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
-    Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-    for (uint32_t m = 0; m < P.split_nud; ++m)
-        cmp_block_sum(dlt, dund, philox_block(STREAM_DIFF | m, ps, pw, rk), P.tdm[2 * m], P.tdm[2 * m + 1], P.sd[2 * m],
-                      P.sd[2 * m + 1]);
-    if (!P.pmask_paper) {
-        for (uint32_t m = 0; m < P.split_nup; ++m)
-            cmp_block_sum(plt, pund, philox_block(STREAM_ANNI | m, ps, pw, rk), P.tpm[2 * m], P.tpm[2 * m + 1], P.sp[2 * m],
-                          P.sp[2 * m + 1]);
-    } else {
-        const U4 pb = philox_block(STREAM_ANNI, ps, pw, rk);
-        const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-        plt.lo = pb.x0 & pb.x2 & gate;
-        plt.hi = pb.x1 & pb.x3 & gate;
-    }
-    uint4 *rec = reinterpret_cast<uint4 *>(P.mask_dev) + (size_t)gw * 96u + lane;
-    rec[0] = make_uint4(misc.x0, misc.x1, y0, misc.x3);
-    rec[32] = make_uint4(dlt.lo, dlt.hi, dund.lo, dund.hi);
-    rec[64] = make_uint4(plt.lo, plt.hi, pund.lo, pund.hi);
+    const uint32_t sigma = __umulhi(philox4x32_10(j / P.A, P.t, 0u, STREAM_SHIFT, P.rk).x0, P.D);  // C5 step 1
+    produce_record(P, task, j, lane, sigma, reinterpret_cast<uint4 *>(P.mask_dev) + (size_t)gw * 96u + lane);
 }
 #endif
 

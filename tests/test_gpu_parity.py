@@ -85,9 +85,11 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
             g.close()
             pytest.skip("libnvrtc is not installed on this box: the built-in kernel ran (and passed the checks above)")
         assert g.jit_state() == 1, pk.jit_message()
-    if expect_split is not None:  # two-kernel small-problem path (mask_kernel + update kernel) or the fused kernel
-        # (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being launched one sweep ahead)
-        assert g.split_launch_count() == (2 * times[-1] + 1 if expect_split else 0)
+    if expect_split is not None:  # which small-problem path ran: launches per handle on the SPLIT paths
+        # True: two-kernel path (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being
+        # launched one sweep ahead); "block": one producer/update block kernel per sweep; False: the fused kernel
+        want = 0 if not expect_split else times[-1] if expect_split == "block" else 2 * times[-1] + 1
+        assert g.split_launch_count() == want
     g.close()
 
 
@@ -136,18 +138,19 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("split", ["auto", "0"])
+@pytest.mark.parametrize("split", ["auto", "0", "block"])
 @pytest.mark.parametrize("case", SMALL, ids=[f"case{i}" for i in range(len(SMALL))])
 def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
     """Every word and count after every sweep.  split = auto: these sizes run the two-kernel small-problem path
     (mask_kernel + update kernel) wherever the warp kernel applies (at most 32 domains per tile); split = 0: the
     fused warp kernel (or the block kernel for more than 32 domains per tile)."""
     variant, L, R, d, p, Ts, D, A, init = case
-    if split == "0":
-        monkeypatch.setenv("PCPD_SPLIT", "0")
+    if split != "auto":
+        monkeypatch.setenv("PCPD_SPLIT", split)
     kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
     warp = min(Ts, L) // D <= 32
-    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)), expect_split=(split == "auto" and warp))
+    gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)),
+              expect_split=(False if split == "0" or not warp else True if split == "auto" else "block"))
 
 
 # cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
@@ -232,6 +235,14 @@ def test_invariants_on_gpu(pk):
     assert np.array_equal(a.get_lattice(), c.get_lattice())
     for h in (a, b, c):
         h.close()
+
+
+def test_mid_size_handle_runs_the_producer_consumer_block_kernel(pk):
+    """Between one tile column per SM and 512 tile columns the default is the one-block producer/consumer form (three
+    producer warps, one update warp, records through a shared-memory ring): sampled columns against the oracle."""
+    L, R = 65536, 64 * 8   # 32 tiles x 8 columns = 256 tile columns
+    kw = dict(L=L, n_replicas=R, d=0.1, p=0.09, seed=2, variant=0)
+    gpu_check(pk, kw, {}, 1, [1, 2, 3], words=[0, 5, 7], expect_split="block")
 
 
 def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
