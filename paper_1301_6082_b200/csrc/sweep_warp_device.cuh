@@ -332,7 +332,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-constexpr uint32_t RING_SLOTS = 12u;   // SPLIT = 3: records in flight between the producer warps and the update warp
+constexpr uint32_t RING_PER_PRODUCER = 4u;   // SPLIT = 3: ring slots (records in flight) per producer warp
 
 }  // namespace
 
@@ -394,13 +394,14 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
     // records when it gets there, and reads each record one attempt ahead of its use.
     const uint32_t nud = SPLIT >= 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT >= 2 ? P.split_nup : (uint32_t)NU_P;
-    // SPLIT = 3 (WPB = 4, ONE tile column per block): warps 1-3 are producers - they compute the records of the
-    // column's attempts (produce_record), attempt j by warp 1 + j mod 3, into a ring of RING_SLOTS records in shared
+    // SPLIT = 3 (ONE tile column per block of WPB warps): warps 1 .. WPB-1 are producers - they compute the records of
+    // the column's attempts (produce_record), attempt j by warp 1 + j mod (WPB-1), into a ring of RING_SLOTS records in shared
     // memory behind the tile - and warp 0 is the update warp.  Per slot a `full` mbarrier (the producer's lane 0
     // arrives once its warp has written the record) and an `empty` one (the update warp's lane 0 arrives once its
     // warp has read it); no global mask buffer, no second kernel.
     uint4 *ring = nullptr;
     uint64_t *fullb = nullptr, *emptyb = nullptr;
+    constexpr uint32_t NPROD = WPB > 1 ? WPB - 1 : 1, RING_SLOTS = RING_PER_PRODUCER * NPROD;
     if constexpr (SPLIT == 3) {
         uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
         ring = reinterpret_cast<uint4 *>(mbase);
@@ -417,7 +418,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         if (warp != 0) {
             const uint32_t J = S * A;
             uint32_t sig = 0u, sig_group = ~0u;   // lane l holds sigma of sub-step 32 * sig_group + l
-            for (uint32_t j = warp - 1u; j < J; j += 3u) {
+            for (uint32_t j = warp - 1u; j < J; j += NPROD) {
                 const uint32_t kk = j / A;
                 if ((kk >> 5) != sig_group) {
                     sig_group = kk >> 5;
