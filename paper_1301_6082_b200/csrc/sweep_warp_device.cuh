@@ -516,6 +516,16 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 
+    uint32_t rslot = 0u, rphase = 0u;   // SPLIT = 3: ring slot and mbarrier phase of the next record to take
+    if constexpr (SPLIT == 3) {
+        mbar_wait(fullb, 0u);
+        const uint4 *r = ring + lane;
+        nx0 = r[0]; nx1 = r[32]; nx2 = r[64];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(emptyb);
+        rslot = 1u % RING_SLOTS;
+        if (RING_SLOTS == 1u) rphase = 1u;
+    }
 #pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
         DomainPos dp{};
@@ -539,12 +549,16 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             U4 blks[1 + NU_D + NU_P];
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
             if constexpr (SPLIT == 3) {
-                const uint32_t j = k * A + a, slot = j % RING_SLOTS, pass = j / RING_SLOTS;
-                mbar_wait(fullb + slot, pass & 1u);
-                const uint4 *r = ring + slot * 96u + lane;
-                const uint4 r0 = r[0], r1 = r[32], r2 = r[64];
-                __syncwarp();
-                if (lane == 0) mbar_arrive(emptyb + slot);
+                // this attempt's record was taken out of the ring during the previous attempt; take the next one now
+                const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
+                if (k * A + a + 1u < S * A) {
+                    mbar_wait(fullb + rslot, rphase);
+                    const uint4 *r = ring + rslot * 96u + lane;
+                    nx0 = r[0]; nx1 = r[32]; nx2 = r[64];
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(emptyb + rslot);
+                    if (++rslot == RING_SLOTS) { rslot = 0u; rphase ^= 1u; }
+                }
                 blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
                 dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
                 plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
