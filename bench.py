@@ -33,9 +33,9 @@ import numpy as np
 import workloads as wl
 
 SWEEPS_PER_STEP = 10
-# dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch from the committed `ncu --set full` capture
-# (profiles/), per config; None where no capture exists.
-NCU_TRAFFIC_BYTES = {"cfg4": 2.091e9}   # profiles/r1d_sweep_kernel_full.md (1.075 GB read + 1.016 GB written per launch)
+# dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, a CONSTANT copied from the committed
+# `ncu --set full` capture named beside it (not measured by this run; re-captured when the kernel changes)
+NCU_TRAFFIC_BYTES = {"cfg4": (2.091e9, "profiles/r1d_sweep_kernel_full.md: 1.075 GB read + 1.016 GB written per launch")}
 METRIC = "replica_site_updates_per_sec"
 UNIT = "replica-site updates/s"
 
@@ -79,18 +79,26 @@ def algorithmic_instr_per_attempt_word(cfg: wl.Config) -> dict:
         lazy = fixed + raw + cmp_blk * lazy_d + (raw + PMASK_PER_BLOCK)
         eager = fixed + raw + cmp_blk * eager_d + (raw + PMASK_PER_BLOCK)
         lazy_blocks, eager_blocks = 2.0 + lazy_d, 2.0 + eager_d
+        cmp_blocks, extra_alu = lazy_d, PMASK_PER_BLOCK
     else:
         lazy_dp = blocks_needed_generic(npd) + blocks_needed_generic(npp)
         eager_dp = (npd + 1) // 2 + (npp + 1) // 2
         lazy = fixed + raw + cmp_blk * lazy_dp
         eager = fixed + raw + cmp_blk * eager_dp
         lazy_blocks, eager_blocks = 1.0 + lazy_dp, 1.0 + eager_dp   # + the MISC block
+        cmp_blocks, extra_alu = lazy_dp, 0.0
+    # the lazy count by pipe (for the three-term bound of SURVEY.md 8(d)): wide multiplies (FMA-heavy pipe, 4 cycles
+    # each), 32-bit IMADs of the generic signed-sum compare (FMA-heavy pipe, 2 cycles each), everything else on the ALU pipe
+    wide = WIDE_FIXED + WIDE_PER_BLOCK * lazy_blocks
+    imad = 0.5 * CMP_PER_BLOCK * cmp_blocks
+    alu = lazy - wide - imad
+    assert abs(alu - (alu_fixed + LOP_PER_BLOCK * lazy_blocks + 0.5 * CMP_PER_BLOCK * cmp_blocks + extra_alu)) < 1e-9
     return dict(lazy=lazy, eager=eager, lazy_blocks=lazy_blocks, eager_blocks=eager_blocks, fixed=fixed,
-                per_block=cmp_blk)
+                per_block=cmp_blk, wide=wide, imad=imad, alu=alu)
 
 
 def variant_name(v: int) -> str:
-    return ("PCPD" if (v & 0xff) == wl.PCPD else "TCPD") + ("+paper-pmask" if v & wl.PMASK_PAPER else "")
+    return {wl.PCPD: "PCPD", wl.TCPD: "TCPD", wl.QCPD: "QCPD", wl.CPD: "CPD"}[v & 0xff] + ("+paper-pmask" if v & wl.PMASK_PAPER else "")
 
 
 def load_peaks() -> dict:
@@ -213,6 +221,91 @@ def reference_arm(args, cfg: wl.Config) -> None:
     print(json.dumps(line), flush=True)
 
 
+# Microbenchmark kinds of the INT peak curve (include/pcpd.h, csrc/microbench.cu): (kind, wide, alu-pipe ops, 32-bit IMAD)
+# per step, for the two pipe models of DESIGN.md section 6.
+PEAK_CURVE = (("lop3", 0, 0, 1, 0), ("imad32", 2, 0, 0, 1), ("wide", 8, 1, 0, 0), ("imad_hi", 6, 1, 0, 0),
+              ("lop3+imad32", 4, 0, 1, 1), ("wide+lop3", 1, 1, 1, 0), ("wide+2lop3", 9, 1, 2, 0), ("wide+3lop3", 5, 1, 3, 0),
+              ("wide+4lop3", 10, 1, 4, 0), ("wide+imad32", 11, 1, 0, 1), ("iadd3", 12, 0, 1, 0),
+              ("wide+lop3+2lop3_one_register", 13, 1, 3, 0), ("wide+lop3+2iadd3", 14, 1, 3, 0),
+              ("2wide+5lop3+imad32", 15, 2, 5, 1))
+
+
+def int_peak_curve(pk, sm_mhz: float) -> dict:
+    """Measured rate of every mix, in lanes per clock per SM, beside what the two pipe models predict: `independent`
+    = ALU pipe (2 cycles per warp-instruction) and FMA-heavy pipe (wide 4, IMAD 2) issue side by side, limited only
+    by one instruction per cycle; `coupled` = a wide multiply also takes 2 cycles of the resource the ALU-pipe
+    instructions use: max(4 W + 2 I, 2 (W + A), W + A + I) cycles per step."""
+    out = {}
+    for name, kind, W, A, I in PEAK_CURVE:
+        rate = pk.microbench(kind, 2000) / 148 / (sm_mhz * 1e6)
+        n = W + A + I
+        indep = 32.0 * 4 * n / max(4 * W + 2 * I, 2 * A, n)
+        coupled = 32.0 * 4 * n / max(4 * W + 2 * I, 2 * (W + A), n)
+        out[name] = dict(kind=kind, lanes_per_clk_per_sm=round(rate, 2), model_independent=round(indep, 1),
+                         model_coupled=round(coupled, 1))
+    return out
+
+
+def kernel_label(h) -> str:
+    return "sweep_warp_kernel" + (" (run-time specialised on T_d, T_p: csrc/jit.cu)" if h.jit_state() == 1
+                                  else " (small-problem paths: launch_ms is per sweep over all its kernels)"
+                                  if h.split_launch_count() > 0 else " (built-in generic-threshold kernel)")
+
+
+def measure_resident(pk, torch, cfg: wl.Config, rank: int, steps: int, warmup: int, barrier, sampler=None) -> dict:
+    """Device-resident timing of one config: `steps` steps of pcpd_run(SWEEPS_PER_STEP) + pcpd_density after `warmup`
+    untimed ones (CUDA events on the launching stream), then the sweep launches alone and the density call alone."""
+    h = pk.Pcpd(cfg.L, cfg.n_replicas, cfg.d, cfg.p, cfg.seed, cfg.variant, word_offset=rank * cfg.W)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record()
+    h.init(cfg.init)
+    ev[1].record()
+    torch.cuda.synchronize()
+    init_ms = ev[0].elapsed_time(ev[1])
+    counts = np.empty(cfg.n_replicas, dtype=np.uint32)
+
+    def step():
+        h.run(SWEEPS_PER_STEP)
+        h.density(counts)
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    l0 = pk.launch_count()
+    if sampler:
+        sampler.start()
+    ev[0].record()
+    for _ in range(steps):
+        step()
+    ev[1].record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = pk.launch_count() - l0
+    t_ms = ev[0].elapsed_time(ev[1])
+    # ---- dominant kernel alone: sweep launch durations ----
+    n_k = max(4, min(40, steps * SWEEPS_PER_STEP))
+    kev = [torch.cuda.Event(enable_timing=True) for _ in range(n_k + 1)]
+    torch.cuda.synchronize()
+    kev[0].record()
+    for i in range(n_k):
+        h.run(1)
+        kev[i + 1].record()
+    torch.cuda.synchronize()
+    sweep_ms = sum(kev[i].elapsed_time(kev[i + 1]) for i in range(n_k)) / n_k
+    ev[2].record()
+    for _ in range(3):
+        h.density(counts)
+    ev[3].record()
+    torch.cuda.synchronize()
+    density_ms = ev[2].elapsed_time(ev[3]) / 3
+    return dict(h=h, t_ms=t_ms, init_ms=init_ms, sweep_ms=sweep_ms, density_ms=density_ms, launches=launches, clocks=clocks)
+
+
+def jit_expected(cfg: wl.Config) -> bool:
+    """Handles with at least 148 x 14 tile columns run the run-time specialised kernel."""
+    return (cfg.L // min(cfg.L, 2048)) * cfg.W >= 148 * 14 and os.environ.get("PCPD_JIT", "1") != "0"
+
+
 def ours_arm(args, cfg: wl.Config) -> None:
     import torch
     import torch.distributed as dist
@@ -239,65 +332,26 @@ def ours_arm(args, cfg: wl.Config) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # weak scaling: every rank owns a cfg-sized shard of word columns of an N x bigger run
-    h = pk.Pcpd(cfg.L, cfg.n_replicas, cfg.d, cfg.p, cfg.seed, cfg.variant, word_offset=rank * cfg.W)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-    ev[0].record()
-    h.init(cfg.init)
-    ev[1].record()
-    torch.cuda.synchronize()
-    init_ms = ev[0].elapsed_time(ev[1])
-    counts = np.empty(cfg.n_replicas, dtype=np.uint32)
-
-    def step():
-        h.run(SWEEPS_PER_STEP)
-        h.density(counts)
-
-    for _ in range(args.warmup):
-        step()
-
-    # ---- timed region 1: device-resident (value) ---------------------------
-    sampler = ClockSampler(local_rank)
-    barrier()
-    l0 = pk.launch_count()
-    sampler.start()
-    ev[0].record()
-    for _ in range(args.steps):
-        step()
-    ev[1].record()
-    barrier()
-    clocks = sampler.stop()
-    launches = pk.launch_count() - l0
-    t_ms = torch.tensor([ev[0].elapsed_time(ev[1])], device="cuda")
+    # ---- timed region 1: device-resident (value); weak scaling: every rank owns a cfg-sized shard of word columns ----
+    m = measure_resident(pk, torch, cfg, rank, args.steps, args.warmup, barrier, ClockSampler(local_rank))
+    h, clocks, launches, sweep_ms, density_ms = m["h"], m["clocks"], m["launches"], m["sweep_ms"], m["density_ms"]
+    if jit_expected(cfg) and h.jit_state() != 1:
+        # a box without NVRTC would silently time the slower built-in kernel: fail loudly instead (PCPD_JIT=0 to allow)
+        raise SystemExit(f"bench.py: {cfg.name} did not get the run-time specialised kernel (jit_state = {h.jit_state()}): "
+                         f"{pk.jit_message()}; set PCPD_JIT=0 to time the built-in kernel on purpose")
+    t_ms = torch.tensor([m["t_ms"]], device="cuda")
     if world > 1:
         dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
     t_ms = float(t_ms.item())
     units_per_step = float(cfg.L) * cfg.n_replicas * SWEEPS_PER_STEP * world
     value = units_per_step * args.steps / (t_ms * 1e-3)
 
-    # ---- dominant kernel alone: sweep kernel launch durations ---------------
-    n_k = max(4, min(40, args.steps * SWEEPS_PER_STEP))
-    kev = [torch.cuda.Event(enable_timing=True) for _ in range(n_k + 1)]
-    torch.cuda.synchronize()
-    kev[0].record()
-    for i in range(n_k):
-        h.run(1)
-        kev[i + 1].record()
-    torch.cuda.synchronize()
-    sweep_ms = sum(kev[i].elapsed_time(kev[i + 1]) for i in range(n_k)) / n_k
-    # density kernel alone
-    ev[2].record()
-    for _ in range(3):
-        h.density(counts)
-    ev[3].record()
-    torch.cuda.synchronize()
-    density_ms = ev[2].elapsed_time(ev[3]) / 3
-
     # ---- timed region 2: end to end through the C ABI with HOST buffers -----
     host_lat = torch.empty((cfg.L, cfg.W), dtype=torch.int64).pin_memory()
     host_cnt = torch.empty(cfg.n_replicas, dtype=torch.int32).pin_memory()
     h.get_lattice_ptr(host_lat.data_ptr())
     e2e_steps = max(2, min(args.steps, 5))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
 
     def e2e_step():
         # one call of the C ABI: H2D of the step's input lattice (cut into column chunks whose copies overlap the
@@ -317,39 +371,74 @@ def ours_arm(args, cfg: wl.Config) -> None:
     if world > 1:
         dist.all_reduce(e_ms, op=dist.ReduceOp.MAX)
     e2e_value = units_per_step * e2e_steps / (float(e_ms.item()) * 1e-3)
+    del host_lat
 
     if rank == 0:
-        alg = algorithmic_instr_per_attempt_word(cfg)
-        attempt_words = float(cfg.L) * cfg.W                      # per sweep launch
         # INT roofline.  Nominal issue peak = 4 schedulers x 32 lanes per SM per clock.  The
-        # kernel's instruction mix (IMAD.WIDE.U32 + ALU-pipe logic) cannot reach it: measured by microbenchmark 5
-        # (one wide multiply + three LOP3 per step, run live here) every instruction of that mix costs 2 issue
-        # cycles per scheduler, i.e. the mix peaks at ~64 lanes/clk/SM.  `peak` is that measured rate.
+        # kernel's instruction mix (IMAD.WIDE.U32 + ALU-pipe logic) cannot reach it: measured by the microbenchmark
+        # curve below (run live here) every instruction of such a mix costs 2 issue cycles per scheduler, i.e. the
+        # mix peaks at ~64 lanes/clk/SM.  `peak` is that measured rate (kind 5: one wide multiply + three LOP3).
         nominal_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6
-        mix_peak = pk.microbench(5, 4000)                          # thread-instr/s, measured on this GPU now
-        achieved = alg["lazy"] * attempt_words / (sweep_ms * 1e-3)
-        hbm_bytes = 2.0 * cfg.lattice_bytes
-        roof = dict(bound="alu", achieved=achieved / 1e12, peak=mix_peak / 1e12, unit="Tinstr/s",
-                    frac=achieved / mix_peak, traffic=NCU_TRAFFIC_BYTES.get(cfg.name),
-                    kernel="sweep_warp_kernel" + (" (run-time specialised on T_d, T_p: csrc/jit.cu)" if h.jit_state() == 1
-                                                  else " (update kernel of the two-kernel small-problem path; launch_ms is "
-                                                       "mask_kernel + update kernel per sweep)" if h.split_launch_count() > 0
-                                                  else " (built-in generic-threshold kernel)"),
-                    launch_ms=sweep_ms,
-                    instr_per_attempt_word=alg["lazy"], lazy_blocks=alg["lazy_blocks"],
-                    frac_eager=alg["eager"] * attempt_words / (sweep_ms * 1e-3) / mix_peak,
-                    frac_of_nominal_issue=achieved / nominal_peak,
+        curve = int_peak_curve(pk, peaks["sm_max_mhz"])
+        to_rate = lambda name: curve[name]["lanes_per_clk_per_sm"] * 148 * peaks["sm_max_mhz"] * 1e6
+        mix_peak, alu_peak, imad_peak, wide_peak = (to_rate(k) for k in ("wide+3lop3", "lop3", "imad32", "wide"))
+
+        def int_roofline(c: wl.Config, launch_ms: float) -> dict:
+            alg = algorithmic_instr_per_attempt_word(c)
+            aw = float(c.L) * c.W                                   # attempt-words per sweep launch
+            achieved = alg["lazy"] * aw / (launch_ms * 1e-3)
+            # SURVEY.md 8(d)'s three-term bound with the measured per-pipe peaks (pipes assumed independent)
+            t_three = aw * max(alg["lazy"] / nominal_peak, alg["alu"] / alu_peak, alg["wide"] / wide_peak + alg["imad"] / imad_peak)
+            hbm = 2.0 * c.lattice_bytes / (launch_ms * 1e-3) / 1e9
+            return dict(alg=alg, achieved=achieved, frac=achieved / mix_peak, frac_three_term=t_three / (launch_ms * 1e-3),
+                        frac_eager=alg["eager"] * aw / (launch_ms * 1e-3) / mix_peak, frac_of_nominal_issue=achieved / nominal_peak,
+                        hbm_gbs=hbm, hbm_frac=hbm / peaks["hbm_gbs"])
+
+        r = int_roofline(cfg, sweep_ms)
+        traffic = NCU_TRAFFIC_BYTES.get(cfg.name)
+        roof = dict(bound="alu", achieved=r["achieved"] / 1e12, peak=mix_peak / 1e12, unit="Tinstr/s", frac=r["frac"],
+                    frac_three_term=r["frac_three_term"],
+                    traffic=traffic[0] if traffic else None,
+                    traffic_source=(traffic[1] + " (constant from that ncu capture, not measured by this run)") if traffic else None,
+                    kernel=kernel_label(h), launch_ms=sweep_ms,
+                    instr_per_attempt_word=r["alg"]["lazy"], lazy_blocks=r["alg"]["lazy_blocks"],
+                    instr_by_pipe=dict(wide=r["alg"]["wide"], imad32=r["alg"]["imad"], alu=r["alg"]["alu"]),
+                    frac_eager=r["frac_eager"], frac_of_nominal_issue=r["frac_of_nominal_issue"],
                     peak_source="measured live: pcpd_microbench(5), IMAD.WIDE.U32 + 3 LOP3 mix on all SMs "
                                 f"({mix_peak / 148 / (peaks['sm_max_mhz'] * 1e6):.1f} lanes/clk/SM); nominal issue peak "
-                                f"148 SMs x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz = {nominal_peak / 1e12:.1f} Tinstr/s",
-                    hbm=dict(achieved=hbm_bytes / (sweep_ms * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
-                             frac=hbm_bytes / (sweep_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], peak_source=peaks["source"]),
+                                f"148 SMs x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz = {nominal_peak / 1e12:.1f} Tinstr/s; "
+                                "frac_three_term = max(N/issue, N_alu/alu_peak, N_wide/wide_peak + N_imad/imad_peak) with "
+                                "the measured single-pipe peaks of int_peak_curve (pipes assumed independent)",
+                    int_peak_curve=curve,
+                    hbm=dict(achieved=r["hbm_gbs"], peak=peaks["hbm_gbs"], unit="GB/s", frac=r["hbm_frac"],
+                             peak_source=peaks["source"]),
                     # the other kernel of the step: positional popcount, reads the lattice once (HBM-bound);
                     # density_ms includes the memset of the counts, their D2H copy and the stream synchronisation
                     density=dict(bound="hbm", achieved=cfg.lattice_bytes / (density_ms * 1e-3) / 1e9,
                                  peak=peaks["hbm_gbs"], unit="GB/s",
                                  frac=cfg.lattice_bytes / (density_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                  call_ms=density_ms))
+        sched = h.schedule_info()
+        h.close()
+        # ---- the other BASELINE.json configs, a few steps each, same step and timing (north_star: "report
+        # throughput on the synthetic configs"); N = 1 only ----
+        configs = {cfg.name: dict(value=value, ms_per_step=t_ms / args.steps, sweep_ms=sweep_ms, frac=r["frac"],
+                                  frac_three_term=r["frac_three_term"], hbm_frac=r["hbm_frac"], kernel=roof["kernel"])}
+        if world == 1 and not args.no_other_configs:
+            for other in wl.CONFIGS:
+                if other.name == cfg.name:
+                    continue
+                mo = measure_resident(pk, torch, other, 0, 5, 3, barrier)
+                ho = mo["h"]
+                if jit_expected(other) and ho.jit_state() != 1:
+                    raise SystemExit(f"bench.py: {other.name} did not get the run-time specialised kernel: {pk.jit_message()}")
+                ro = int_roofline(other, mo["sweep_ms"])
+                configs[other.name] = dict(value=float(other.L) * other.n_replicas * SWEEPS_PER_STEP * 5 / (mo["t_ms"] * 1e-3),
+                                           ms_per_step=mo["t_ms"] / 5, sweep_ms=mo["sweep_ms"], frac=ro["frac"],
+                                           frac_three_term=ro["frac_three_term"], hbm_frac=ro["hbm_frac"],
+                                           kernel=kernel_label(ho), steps=5, warmup=3,
+                                           l2="lattice larger than L2" if other.lattice_bytes > 200e6 else "lattice smaller than L2")
+                ho.close()
         cores = max(1, min(os.cpu_count() or 1, cfg.W, 16))
         L_sample = min(cfg.L, 1 << 17)
         _, dt1 = oracle_sample_rate(cfg, L_sample, cores, 1)         # calibration sweep
@@ -363,11 +452,11 @@ def ours_arm(args, cfg: wl.Config) -> None:
                     config=dict(workload=cfg.name, L=cfg.L, n_replicas=cfg.n_replicas, d=cfg.d, p=cfg.p,
                                 variant=variant_name(cfg.variant), seed=cfg.seed,
                                 sweeps_per_step=SWEEPS_PER_STEP, step="pcpd_run(10) + pcpd_density",
-                                schedule=h.schedule_info(), lattice_bytes=cfg.lattice_bytes,
+                                schedule=sched, lattice_bytes=cfg.lattice_bytes,
                                 l2="lattice (1 GiB at cfg4) is larger than L2; no flush needed" if cfg.lattice_bytes > 200e6
                                 else "lattice smaller than L2 (correctness config)",
-                                init_ms=init_ms, density_ms=density_ms, parallelism=f"replica-word shards x{world}"),
-                    roofline=roof,
+                                init_ms=m["init_ms"], density_ms=density_ms, parallelism=f"replica-word shards x{world}"),
+                    roofline=roof, configs=configs,
                     cpu_baseline=dict(value=cpu_rate, unit=UNIT, cores=cores, kind="oracle", sample=sample,
                                       lazy_blocks_per_attempt_word=LAST_ORACLE_LAZY_BLOCKS),
                     e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=cfg.lattice_bytes,
@@ -375,7 +464,8 @@ def ours_arm(args, cfg: wl.Config) -> None:
                              call="pcpd_step_from_host(host lattice, 10 sweeps, host counts)"),
                     gpu_launches=int(launches), clocks=clocks)
         print(json.dumps(line), flush=True)
-    h.close()
+    else:
+        h.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -387,6 +477,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg4", choices=sorted(wl.BY_NAME))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short runs of the other BASELINE configs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = wl.BY_NAME[args.config]

@@ -86,7 +86,9 @@ enum pcpd_init_mode { PCPD_INIT_FULL = 0, PCPD_INIT_BERNOULLI = 1, PCPD_INIT_EMP
  * Optional.  alloc(bytes, stream) returns a DEVICE pointer (NULL on failure),
  * release(ptr) frees it.  The Python binding installs PyTorch's CUDA caching
  * allocator here; without it the library uses cudaMalloc/cudaFree.  Process
- * wide; call before pcpd_create. */
+ * wide; every handle remembers the pair it was created with and frees its buffers
+ * through it.  PCPD_ERR_ARG while any handle is alive, or if only one of the two is given.
+ * Thread-safe, like pcpd_create* (first-use configuration of a device is serialised). */
 typedef void *(*pcpd_alloc_fn)(size_t bytes, void *cuda_stream);
 typedef void (*pcpd_free_fn)(void *dev_ptr);
 PCPD_API int pcpd_set_allocator(pcpd_alloc_fn alloc, pcpd_free_fn release);
@@ -120,8 +122,9 @@ PCPD_API pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, doubl
  * handle (global column word_offset + w) uses d_w[w], p_w[w] - HOST arrays of n_replicas/64 doubles, copied at
  * create time - instead of one (d, p); everything else is as in pcpd_create_ex, and column w evolves bit for bit
  * as it would in a uniform run with (d_w[w], p_w[w]).  Errors as pcpd_create_ex, plus: NULL arrays, any entry
- * outside [0,1] or NaN, the PCPD_VARIANT_PMASK_PAPER flag (not available in this mode), more than 32 domains per
- * tile (T_s / D > 32).  pcpd_thresholds reports column 0's thresholds. */
+ * outside [0,1] or NaN, the PCPD_VARIANT_PMASK_PAPER flag (not available in this mode), a schedule the
+ * warp-per-tile-column kernel cannot run (more than 32 domains per tile, T_s / D > 32, or a tile column above
+ * 200 KiB, T_s > 25598).  pcpd_thresholds reports column 0's thresholds. */
 PCPD_API pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, const double *p_w, uint64_t seed,
                          int variant, uint32_t T_s, uint32_t D, uint32_t A, uint64_t word_offset);
 
@@ -139,8 +142,10 @@ PCPD_API int pcpd_run(pcpd_t *h, uint64_t n_sweeps);
  * the caller's division), r < n_replicas.  Synchronises the stream. */
 PCPD_API int pcpd_density(pcpd_t *h, uint32_t *out_counts);
 
-/* out_pairs[r] = number of adjacent occupied pairs sum_i q(i) q(i+1) of
- * replica r (pair density of PAPER.md:203-208, Figs 5-6).  Synchronises. */
+/* out_pairs[r] = number of adjacent occupied pairs sum_i q(i) q(next(i)) whose left site lies in
+ * replica lane r (pair density of PAPER.md:203-208, Figs 5-6).  Independent replicas: next(L-1) =
+ * site 0 of the same lane.  PCPD_VARIANT_CONNECTED: next(site L-1, lane j) = (site 0, lane j+1 mod 64)
+ * of the same word column, so 64 consecutive entries sum to the pair count of that ring.  Synchronises. */
 PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
 
 /* A whole time series in one call (the paper's observable is rho(t) at many times, Fig. 1; pair
@@ -151,6 +156,18 @@ PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
  * device until the end: one read-back and one synchronisation for the series instead of one per record.
  * PCPD_ERR_ARG for non-ascending times, PCPD_ERR_RANGE past 2^32 - 1; on error the counter stays where it got to. */
 PCPD_API int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs);
+
+/* Effective exponent of a density series (host-side analysis; eq. (2) and Figs 5-6:
+ * "a straight line is obtained by plotting delta_eff as a function of rho"):
+ *     rho[k]   = mean over the n_replicas replicas of series[k*n_replicas + r] / L
+ *     delta[k] = - ln(rho[k+m] / rho[k-m]) / ln(times[k+m] / times[k-m]),   m = half_window >= 1
+ * i.e. delta_eff = -d ln rho / d ln t as a central difference in log-log coordinates.  `series` is what
+ * pcpd_run_series wrote (particle counts or pair counts), `times` the sweep indices it was given.  out_rho,
+ * out_delta: n_times doubles each; delta[k] is NaN where the window does not fit, where a time in it is 0 or
+ * repeated, or where a density in it is 0.  Plain host arithmetic in double; no device is touched.
+ * PCPD_ERR_ARG for NULL pointers, n_times == 0, n_replicas == 0, L == 0, half_window == 0 or descending times. */
+PCPD_API int pcpd_delta_eff(const uint64_t *times, uint64_t n_times, const uint32_t *series, uint64_t n_replicas,
+                            uint64_t L, uint32_t half_window, double *out_rho, double *out_delta);
 
 /* Lattice in canonical order words[i*W + w], L*W uint64.  Synchronise. */
 PCPD_API int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words);
@@ -231,6 +248,10 @@ PCPD_API uint64_t pcpd_launch_count(void);
  * independent chains (do the ALU and FMA pipes co-issue?); 5: IMAD.WIDE.U32 + 3 LOP3
  * (the sweep kernel's mix: bench.py's roofline peak); 6: IMAD.HI.U32 only;
  * 7: Philox with mul.hi + mad.lo written separately (ptxas fuses them back).
+ * Kinds 8 .. 15 are the curve behind the roofline peak (rate = instructions as written):
+ * 8: IMAD.WIDE.U32 only; 9: wide : LOP3 = 1 : 2; 10: 1 : 4; 11: wide + 32-bit IMAD 1 : 1;
+ * 12: IADD3 only; 13: wide + 3 LOP3 of which two read ONE register (and an immediate);
+ * 14: wide + LOP3 + 2 IADD3; 15: 2 wide : 5 LOP3 : 1 IMAD (the sweep kernel's own mix).
  * PCPD_ERR_ARG for another kind, iters == 0 or a NULL out pointer. */
 PCPD_API int pcpd_microbench(int kind, uint32_t iters, double *out_rate);
 

@@ -29,8 +29,13 @@
  *   oracle_set_word_probabilities  P11 column k of a per-word run == column k of the uniform
  *                                 run with (d_k, p_k), bit for bit
  *   oracle_run (schedule SD2) P5  vs literal Alg. 1 (statistical), P6 exact toy
- *                                 operator, P7 run splitting / loop order /
- *                                 word subsets
+ *                                 operator (all four rules), P7 run splitting / loop
+ *                                 order / word subsets
+ *   oracle_counts / oracle_pair_counts  P7  numpy column popcounts incl. the ring closure
+ *                                 (independent lanes: site L-1 -> 0; connected lattice:
+ *                                 the unrolled ring of 64 L sites)
+ *   planes_needed / oracle_stats  P12 brute-force "first differing plane" per lane from the
+ *                                 pinned lane uniforms; closed form sum_m [1-(1-4^-m)^64]
  * Parity status: every function pinned; the *numerical values* of rho(t) at the
  * five configs are "parity unpinned by the paper" (it prints none).
  */
@@ -524,13 +529,20 @@ void oracle_counts(const oracle_t *o, uint32_t *out)
     }
 }
 
-/* pair count: sum_i q(i) q(i+1). */
+/* pair count: out[r] = sum_i q_r(i) q_next(i), the number of
+ * adjacent occupied pairs whose LEFT site lies in replica lane r.  Independent replicas: the ring
+ * closes inside the lane, next(L-1) = site 0 of the same lane.  Connected multispin lattice (C10,
+ * PAPER.md:98-100, 118): the 64 lanes of a word column are consecutive segments of one ring of
+ * 64 L sites, so the right neighbour of (site L-1, lane j) is (site 0, lane (j+1) mod 64) of the
+ * same word column; the sum over a column's 64 lanes is then the pair count of that ring. */
 void oracle_pair_counts(const oracle_t *o, uint32_t *out)
 {
     for (uint32_t r = 0; r < o->nwords * 64; ++r) {
         uint32_t cnt = 0;
         const uint8_t *q = o->q + (size_t)r * o->L;
-        for (uint32_t i = 0; i < o->L; ++i) cnt += (uint32_t)(q[i] & q[(i + 1) % o->L]);
+        for (uint32_t i = 0; i + 1 < o->L; ++i) cnt += (uint32_t)(q[i] & q[i + 1]);
+        uint32_t rn = o->connected ? (r / 64) * 64 + (r % 64 + 1) % 64 : r;   /* lane holding the successor of site L-1 */
+        cnt += (uint32_t)(q[o->L - 1] & o->q[(size_t)rn * o->L]);
         out[r] = cnt;
     }
 }

@@ -34,7 +34,7 @@ EXPORTS = (
     "pcpd_density", "pcpd_pair_density", "pcpd_get_lattice", "pcpd_set_lattice", "pcpd_schedule_info",
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
-    "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host", "pcpd_run_series",
+    "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host", "pcpd_run_series", "pcpd_delta_eff",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -124,6 +124,8 @@ def load_library() -> C.CDLL:
     L.pcpd_step_from_host.restype = C.c_int
     L.pcpd_split_launch_count.argtypes = [C.c_void_p]
     L.pcpd_split_launch_count.restype = C.c_uint64
+    L.pcpd_delta_eff.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
+    L.pcpd_delta_eff.restype = C.c_int
     _lib = L
     return L
 
@@ -183,6 +185,21 @@ def microbench(kind: int, iters: int = 2000) -> float:
     out = C.c_double()
     _check(L, L.pcpd_microbench(kind, iters, C.byref(out)))
     return out.value
+
+
+def delta_eff(times, series, L, half_window=1):
+    """pcpd_delta_eff: (rho[k], delta_eff[k]) of a density series: rho = mean count / L,
+    delta_eff = -d ln rho / d ln t as a central log-log difference over +- half_window records (NaN at the ends).
+    `series` is counts[len(times), n_replicas] as pcpd_run_series returns it (particle or pair counts)."""
+    lib = load_library()
+    t = np.ascontiguousarray(times, dtype=np.uint64)
+    c = np.ascontiguousarray(series, dtype=np.uint32)
+    if c.ndim != 2 or c.shape[0] != len(t):
+        raise ValueError("series must be counts[len(times), n_replicas]")
+    rho, dl = np.empty(len(t)), np.empty(len(t))
+    _check(lib, lib.pcpd_delta_eff(t.ctypes.data, len(t), c.ctypes.data, c.shape[1], int(L), int(half_window),
+                                   rho.ctypes.data, dl.ctypes.data))
+    return rho, dl
 
 
 class Pcpd:

@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <atomic>
+#include <mutex>
 #include <new>
 
 #include "../../include/pcpd.h"
@@ -18,9 +19,14 @@ namespace {
 
 thread_local char g_err[512] = "";
 std::atomic<uint64_t> g_launches{0};
+// Process-wide state, guarded by g_mu: the allocator pair new handles will use, the number of live handles (the pair
+// cannot be swapped under them) and the per-device first-use configuration (the opt-in shared-memory attribute is per
+// context).  Everything else a call touches belongs to its handle.
+std::mutex g_mu;
 pcpd_alloc_fn g_alloc = nullptr;
 pcpd_free_fn g_free = nullptr;
-bool g_configured[64] = {};  // per device: the opt-in shared-memory attribute is per context
+uint64_t g_live = 0;
+bool g_configured[64] = {};
 
 int fail(int code, const char *fmt, ...)
 {
@@ -36,9 +42,15 @@ int cuda_fail(cudaError_t e, const char *what)
     return fail(PCPD_ERR_DEVICE, "%s: %s", what, cudaGetErrorString(e));
 }
 
-void *dev_alloc(size_t bytes, cudaStream_t s)
+// device memory through the allocator pair the handle was created with (NULL pair: cudaMalloc / cudaFree)
+struct Allocator {
+    pcpd_alloc_fn alloc;
+    pcpd_free_fn release;
+};
+
+void *dev_alloc(const Allocator &a, size_t bytes, cudaStream_t s)
 {
-    if (g_alloc) return g_alloc(bytes, (void *)s);
+    if (a.alloc) return a.alloc(bytes, (void *)s);
     void *p = nullptr;
     if (cudaMalloc(&p, bytes) != cudaSuccess) {
         cudaGetLastError();
@@ -47,10 +59,10 @@ void *dev_alloc(size_t bytes, cudaStream_t s)
     return p;
 }
 
-void dev_free(void *p)
+void dev_free(const Allocator &a, void *p)
 {
     if (!p) return;
-    if (g_free) g_free(p);
+    if (a.release) a.release(p);
     else cudaFree(p);
 }
 
@@ -76,17 +88,45 @@ struct pcpd_s {
     uint32_t Ts, D, A;
     uint64_t word_offset;
     uint64_t Td, Tp;
-    int Wb;
     uint64_t sweep;
     bool force_block;  // test hook (env PCPD_FORCE_BLOCK_KERNEL=1 at create): run the generic block kernel
+    bool invalid;      // a pipelined pcpd_step_from_host failed part-way: the lattice is undefined until set_lattice / init
+    int connected;     // PCPD_VARIANT_CONNECTED
+    Allocator mem;     // the allocator pair in force when the handle was created
     uint32_t *thr;     // device, per-word thresholds [W][4] (pcpd_create_scan), else NULL
-    uint64_t *lat;     // device, word-blocked
+    uint64_t *lat;     // device, column-major [W][L]
     uint32_t *counts;  // device, uint32[R]
     cudaStream_t stream;
     SweepParams P;
     JitSlot jit;       // threshold-specialised sweep kernel (jit.cu); mode from env PCPD_JIT at create
     SplitSlot split;   // small problems: mask buffer of the two-kernel sweep (sweep_warp.cu); env PCPD_SPLIT
+    // pcpd_step_from_host: copy stream and events, created on first use and kept for the life of the handle
+    cudaStream_t copy_stream;
+    cudaEvent_t copy_start;
+    cudaEvent_t *chunk_ev;
+    uint32_t n_chunk_ev;
 };
+
+static void release_handle(pcpd_s *h)   // frees everything the handle owns (partially constructed handles too)
+{
+    split_teardown(&h->split);
+    if (h->copy_stream) {
+        cudaStreamSynchronize(h->copy_stream);
+        cudaStreamDestroy(h->copy_stream);
+    }
+    if (h->copy_start) cudaEventDestroy(h->copy_start);
+    for (uint32_t c = 0; c < h->n_chunk_ev; ++c)
+        if (h->chunk_ev[c]) cudaEventDestroy(h->chunk_ev[c]);
+    delete[] h->chunk_ev;
+    dev_free(h->mem, h->thr);
+    dev_free(h->mem, h->split.buf[0]);
+    dev_free(h->mem, h->split.buf[1]);
+    dev_free(h->mem, h->lat);
+    dev_free(h->mem, h->counts);
+    delete h;
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g_live) --g_live;
+}
 
 extern "C" {
 
@@ -96,6 +136,9 @@ uint64_t pcpd_launch_count(void) { return g_launches.load(); }
 int pcpd_set_allocator(pcpd_alloc_fn alloc, pcpd_free_fn release)
 {
     if ((alloc == nullptr) != (release == nullptr)) return fail(PCPD_ERR_ARG, "set_allocator: give both or neither");
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g_live && (alloc != g_alloc || release != g_free))
+        return fail(PCPD_ERR_ARG, "set_allocator: %llu handle(s) are alive; destroy them first", (unsigned long long)g_live);
     g_alloc = alloc;
     g_free = release;
     return PCPD_OK;
@@ -151,19 +194,18 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_ARG, "schedule: D / A must be <= %u", MAX_SUBSTEPS);
         return nullptr;
     }
-    // Physical layout: column-major [W][L] (word-group width Wb = 1): a tile column is one
-    // contiguous run of T_s words, which is what the warp-per-(tile, column) sweep kernel loads.
-    const int Wb = 1;
+    // Physical layout: column-major [W][L]: a tile column is one contiguous run of T_s words, which is
+    // what the warp-per-(tile, column) sweep kernel loads.
     if (pmask_paper && !sweep_warp_supported(Ts, D)) {
         fail(PCPD_ERR_ARG, "the paper's annihilation mask needs at most 32 domains per tile (T_s / D <= 32)");
         return nullptr;
     }
-    if (!sweep_warp_supported(Ts, D) && (sweep_smem_bytes(Ts, Wb) > 200 * 1024 || (uint64_t)(Ts / D) > 1024)) {
+    if (!sweep_warp_supported(Ts, D) && (sweep_smem_bytes(Ts) > 200 * 1024 || (uint64_t)(Ts / D) > 1024)) {
         fail(PCPD_ERR_ARG, "schedule: tile of %u sites does not fit one thread block", Ts);
         return nullptr;
     }
-    if (W / Wb > 65535) {
-        fail(PCPD_ERR_ARG, "too many word columns for one handle (W / %d > 65535): shard by word_offset", Wb);
+    if (W > 65535) {
+        fail(PCPD_ERR_ARG, "too many word columns for one handle (W > 65535): shard by word_offset");
         return nullptr;
     }
 
@@ -183,27 +225,37 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_DEVICE, "device index %d out of range", dev);
         return nullptr;
     }
-    if (!g_configured[dev]) {
-        const int rc = configure_kernels();
-        if (rc != 0) {
-            cuda_fail((cudaError_t)rc, "cudaFuncSetAttribute");
-            return nullptr;
-        }
-        g_configured[dev] = true;
-    }
-
     pcpd_s *h = new (std::nothrow) pcpd_s();
     if (!h) {
         fail(PCPD_ERR_ALLOC, "host allocation failed");
         return nullptr;
     }
+    {
+        // first use of a device configures the kernels (opt-in shared memory); serialised, as is the snapshot of
+        // the allocator pair this handle will allocate and free with
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (!g_configured[dev]) {
+            const int rc = configure_kernels();
+            if (rc != 0) {
+                delete h;
+                cuda_fail((cudaError_t)rc, "cudaFuncSetAttribute");
+                return nullptr;
+            }
+            g_configured[dev] = true;
+        }
+        h->mem = Allocator{g_alloc, g_free};
+        ++g_live;
+    }
     h->L = L; h->R = n_replicas; h->W = W; h->d = d; h->p = p; h->seed = seed; h->variant = variant;
-    h->Ts = Ts; h->D = D; h->A = A; h->word_offset = word_offset; h->Wb = Wb; h->sweep = 0;
+    h->Ts = Ts; h->D = D; h->A = A; h->word_offset = word_offset; h->sweep = 0;
     h->Td = threshold_of(d); h->Tp = threshold_of(p);
+    h->invalid = false;
+    h->connected = connected;
+    h->copy_stream = nullptr; h->copy_start = nullptr; h->chunk_ev = nullptr; h->n_chunk_ev = 0;
     {
         const char *fb = getenv("PCPD_FORCE_BLOCK_KERNEL");
         h->force_block = fb && fb[0] == '1' && !pmask_paper && (uint64_t)(Ts / D) <= 1024 &&
-                         sweep_smem_bytes(Ts, Wb) <= 200 * 1024;
+                         sweep_smem_bytes(Ts) <= 200 * 1024;
     }
     {
         const char *jm = getenv("PCPD_JIT");  // unset / "1": auto (large problems); "0": off; "force": every size
@@ -215,12 +267,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     memset(&h->split, 0, sizeof h->split);
     h->stream = nullptr;
     h->thr = nullptr;
-    h->lat = (uint64_t *)dev_alloc(8 * L * W, h->stream);
-    h->counts = (uint32_t *)dev_alloc(4 * n_replicas, h->stream);
+    h->lat = (uint64_t *)dev_alloc(h->mem, 8 * L * W, h->stream);
+    h->counts = (uint32_t *)dev_alloc(h->mem, 4 * n_replicas, h->stream);
     if (!h->lat || !h->counts) {
-        dev_free(h->lat);
-        dev_free(h->counts);
-        delete h;
+        release_handle(h);
         fail(PCPD_ERR_ALLOC, "device allocation of %llu bytes failed", (unsigned long long)(8 * L * W));
         return nullptr;
     }
@@ -267,13 +317,13 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         const size_t bytes = split_mask_bytes(P);
         if (mode && mode != 3 && split_supported(Ts, D) && !h->force_block &&
             (mode == 2 ? bytes <= (1ull << 30) : ntasks <= (uint64_t)prop.multiProcessorCount)) {
-            h->split.buf[0] = dev_alloc(bytes, h->stream);   // any failure here: the fused kernel is used
-            h->split.buf[1] = h->split.buf[0] ? dev_alloc(bytes, h->stream) : nullptr;
+            h->split.buf[0] = dev_alloc(h->mem, bytes, h->stream);   // any failure here: the fused kernel is used
+            h->split.buf[1] = h->split.buf[0] ? dev_alloc(h->mem, bytes, h->stream) : nullptr;
             if (!h->split.buf[1] || split_setup(&h->split) != 0) {
                 cudaGetLastError();
                 split_teardown(&h->split);
-                dev_free(h->split.buf[0]);
-                dev_free(h->split.buf[1]);
+                dev_free(h->mem, h->split.buf[0]);
+                dev_free(h->mem, h->split.buf[1]);
                 h->split.buf[0] = h->split.buf[1] = nullptr;
             }
         }
@@ -309,14 +359,16 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
                  (unsigned long long)w);
             return nullptr;
         }
-    if (Ts == 0 || D == 0 || (uint64_t)((Ts > L ? L : Ts) / D) > 32) {
-        fail(PCPD_ERR_ARG, "create_scan needs at most 32 domains per tile (T_s / D <= 32)");
+    // per-word thresholds exist in the warp-per-tile-column kernel only: the schedule must be one it can run
+    if (Ts == 0 || D == 0 || !sweep_warp_supported((uint32_t)(Ts > L ? L : Ts), D)) {
+        fail(PCPD_ERR_ARG, "create_scan needs at most 32 domains per tile (T_s / D <= 32) and a tile column of at most "
+                           "200 KiB (T_s <= 25598)");
         return nullptr;
     }
     pcpd_t *h = pcpd_create_ex(L, n_replicas, d_w[0], p_w[0], seed, variant, Ts, D, A, word_offset);
     if (!h) return nullptr;
     uint32_t *host = new (std::nothrow) uint32_t[4 * W];
-    h->thr = (uint32_t *)dev_alloc(16 * W, h->stream);
+    h->thr = (uint32_t *)dev_alloc(h->mem, 16 * W, h->stream);
     if (!host || !h->thr) {
         delete[] host;
         pcpd_destroy(h);
@@ -341,8 +393,8 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
     h->force_block = false;
     h->split.block_mode = 0;
     split_teardown(&h->split);   // per-word thresholds run the fused kernel
-    dev_free(h->split.buf[0]);
-    dev_free(h->split.buf[1]);
+    dev_free(h->mem, h->split.buf[0]);
+    dev_free(h->mem, h->split.buf[1]);
     h->split.buf[0] = h->split.buf[1] = nullptr;
     return h;
 }
@@ -351,13 +403,7 @@ void pcpd_destroy(pcpd_t *h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
-    split_teardown(&h->split);
-    dev_free(h->thr);
-    dev_free(h->split.buf[0]);
-    dev_free(h->split.buf[1]);
-    dev_free(h->lat);
-    dev_free(h->counts);
-    delete h;
+    release_handle(h);
 }
 
 int pcpd_set_stream(pcpd_t *h, void *cuda_stream)
@@ -366,6 +412,9 @@ int pcpd_set_stream(pcpd_t *h, void *cuda_stream)
     h->stream = (cudaStream_t)cuda_stream;
     return PCPD_OK;
 }
+
+static const char kInvalidMsg[] =
+    "the handle's lattice is undefined (a pipelined pcpd_step_from_host failed part-way): call pcpd_set_lattice or pcpd_init";
 
 static int check_launch(const char *what)
 {
@@ -378,19 +427,22 @@ int pcpd_init(pcpd_t *h, int mode)
 {
     if (!h) return fail(PCPD_ERR_ARG, "null handle");
     if (mode < 0 || mode > 2) return fail(PCPD_ERR_ARG, "unknown init mode %d", mode);
-    g_launches += launch_init(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, (uint32_t)h->word_offset, mode, h->P.rk,
-                              h->stream);
+    g_launches += launch_init(h->lat, (uint32_t)h->L, (uint32_t)h->W, (uint32_t)h->word_offset, mode, h->P.rk, h->stream);
     h->sweep = 0;
+    h->invalid = false;
     return check_launch("init kernel");
 }
 
 int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
 {
     if (!h) return fail(PCPD_ERR_ARG, "null handle");
+    if (h->invalid) return fail(PCPD_ERR_DEVICE, "%s", kInvalidMsg);
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit, &h->split);
+        const int nl = launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit, &h->split);
+        if (nl < 0) return cuda_fail(cudaGetLastError(), "sweep launch (stream / event operation of the two-kernel path)");
+        g_launches += nl;
         h->sweep += 1;
     }
     return check_launch("sweep kernel");
@@ -399,9 +451,10 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
 static int density_impl(pcpd_t *h, uint32_t *out, int pairs)
 {
     if (!h || !out) return fail(PCPD_ERR_ARG, "null argument");
+    if (h->invalid) return fail(PCPD_ERR_DEVICE, "%s", kInvalidMsg);
     cudaError_t e = cudaMemsetAsync(h->counts, 0, 4 * h->R, h->stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset");
-    g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, pairs, h->counts, h->stream);
+    g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, pairs, h->connected, h->counts, h->stream);
     int rc = check_launch("density kernel");
     if (rc) return rc;
     e = cudaMemcpyAsync(out, h->counts, 4 * h->R, cudaMemcpyDeviceToHost, h->stream);
@@ -422,7 +475,7 @@ int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t
     }
     const int nobs = (out_counts ? 1 : 0) + (out_pairs ? 1 : 0);
     const size_t row = 4 * h->R, bytes = row * n_times * nobs;
-    uint32_t *series = (uint32_t *)dev_alloc(bytes, h->stream);
+    uint32_t *series = (uint32_t *)dev_alloc(h->mem, bytes, h->stream);
     if (!series) return fail(PCPD_ERR_ALLOC, "run_series: allocation of %llu bytes failed", (unsigned long long)bytes);
     cudaError_t e = cudaMemsetAsync(series, 0, bytes, h->stream);
     int rc = PCPD_OK;
@@ -430,9 +483,10 @@ int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t
         rc = pcpd_run(h, times[k] - h->sweep);
         if (rc != PCPD_OK) break;
         uint32_t *dst = series + (size_t)k * h->R * nobs;   // record k: [counts][pairs]
-        if (out_counts) g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 0, dst, h->stream);
+        if (out_counts) g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, 0, 0, dst, h->stream);
         if (out_pairs)
-            g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 1, dst + (out_counts ? h->R : 0), h->stream);
+            g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, 1, h->connected, dst + (out_counts ? h->R : 0),
+                                         h->stream);
         rc = check_launch("density kernel");
     }
     // ONE read-back and ONE synchronisation for the whole series
@@ -446,31 +500,57 @@ int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t
         }
     }
     const cudaError_t es = cudaStreamSynchronize(h->stream);
-    dev_free(series);
+    dev_free(h->mem, series);
     if (rc != PCPD_OK) return rc;
     if (e == cudaSuccess) e = es;
     if (e != cudaSuccess) return cuda_fail(e, "run_series");
     return PCPD_OK;
 }
 
+int pcpd_delta_eff(const uint64_t *times, uint64_t n_times, const uint32_t *series, uint64_t n_replicas, uint64_t L,
+                   uint32_t half_window, double *out_rho, double *out_delta)
+{
+    if (!times || !series || !out_rho || !out_delta || n_times == 0 || n_replicas == 0 || L == 0 || half_window == 0)
+        return fail(PCPD_ERR_ARG, "delta_eff: null or zero argument");
+    for (uint64_t k = 1; k < n_times; ++k)
+        if (times[k] < times[k - 1]) return fail(PCPD_ERR_ARG, "delta_eff: times must ascend");
+    for (uint64_t k = 0; k < n_times; ++k) {
+        uint64_t sum = 0;   // exact: at most 2^32 replicas x counts below 2^32
+        for (uint64_t r = 0; r < n_replicas; ++r) sum += series[k * n_replicas + r];
+        out_rho[k] = (double)sum / ((double)n_replicas * (double)L);
+    }
+    const uint64_t m = half_window;
+    for (uint64_t k = 0; k < n_times; ++k) {
+        double v = std::nan("");
+        if (k >= m && k + m < n_times) {
+            const uint64_t t0 = times[k - m], t1 = times[k + m];
+            const double r0 = out_rho[k - m], r1 = out_rho[k + m];
+            if (t0 > 0 && t1 > t0 && r0 > 0.0 && r1 > 0.0) v = -std::log(r1 / r0) / std::log((double)t1 / (double)t0);
+        }
+        out_delta[k] = v;
+    }
+    return PCPD_OK;
+}
+
 int pcpd_get_lattice(pcpd_t *h, uint64_t *out_words)
 {
     if (!h || !out_words) return fail(PCPD_ERR_ARG, "null argument");
+    if (h->invalid) return fail(PCPD_ERR_DEVICE, "%s", kInvalidMsg);
     const size_t bytes = 8 * h->L * h->W;
     cudaError_t e;
-    if ((uint64_t)h->Wb == h->W) {  // single word group: physical == canonical
+    if (h->W == 1) {  // a single column: device layout == canonical
         e = cudaMemcpyAsync(out_words, h->lat, bytes, cudaMemcpyDeviceToHost, h->stream);
     } else {
-        uint64_t *tmp = (uint64_t *)dev_alloc(bytes, h->stream);
+        uint64_t *tmp = (uint64_t *)dev_alloc(h->mem, bytes, h->stream);
         if (!tmp) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
-        g_launches += launch_permute(h->lat, tmp, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 0, h->stream);
+        g_launches += launch_transpose(h->lat, tmp, (uint32_t)h->L, (uint32_t)h->W, 0, h->stream);
         e = cudaMemcpyAsync(out_words, tmp, bytes, cudaMemcpyDeviceToHost, h->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-        dev_free(tmp);
+        dev_free(h->mem, tmp);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(e, "get_lattice");
-    return check_launch("permute kernel");
+    return check_launch("transpose kernel");
 }
 
 int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words)
@@ -478,19 +558,21 @@ int pcpd_set_lattice(pcpd_t *h, const uint64_t *in_words)
     if (!h || !in_words) return fail(PCPD_ERR_ARG, "null argument");
     const size_t bytes = 8 * h->L * h->W;
     cudaError_t e;
-    if ((uint64_t)h->Wb == h->W) {
+    if (h->W == 1) {
         e = cudaMemcpyAsync(h->lat, in_words, bytes, cudaMemcpyHostToDevice, h->stream);
     } else {
-        uint64_t *tmp = (uint64_t *)dev_alloc(bytes, h->stream);
+        uint64_t *tmp = (uint64_t *)dev_alloc(h->mem, bytes, h->stream);
         if (!tmp) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
         e = cudaMemcpyAsync(tmp, in_words, bytes, cudaMemcpyHostToDevice, h->stream);
-        g_launches += launch_permute(tmp, h->lat, (uint32_t)h->L, (uint32_t)h->W, h->Wb, 1, h->stream);
+        g_launches += launch_transpose(tmp, h->lat, (uint32_t)h->L, (uint32_t)h->W, 1, h->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-        dev_free(tmp);
+        dev_free(h->mem, tmp);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(e, "set_lattice");
-    return check_launch("permute kernel");
+    const int rc = check_launch("transpose kernel");
+    if (rc == PCPD_OK) h->invalid = false;
+    return rc;
 }
 
 // Column chunk of the pipelined step: 8 word columns (64-byte rows of the canonical host layout) when the handle has
@@ -519,19 +601,32 @@ int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, 
         return rc;
     }
     const size_t bytes = 8 * h->L * h->W;
-    uint64_t *stage = (uint64_t *)dev_alloc(bytes, h->stream);
-    if (!stage) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
-    cudaStream_t copy = nullptr;
-    cudaError_t e = cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking);
     const uint32_t nchunks = (W + cw - 1) / cw;
-    cudaEvent_t *ev = new (std::nothrow) cudaEvent_t[nchunks]();
-    cudaEvent_t start = nullptr;
-    if (e == cudaSuccess && !ev) e = cudaErrorMemoryAllocation;
-    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) e = cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming);
+    // copy stream and events: created on first use, kept for the life of the handle
+    cudaError_t e = cudaSuccess;
+    if (!h->copy_stream) e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess && !h->copy_start) e = cudaEventCreateWithFlags(&h->copy_start, cudaEventDisableTiming);
+    if (e == cudaSuccess && h->n_chunk_ev < nchunks) {
+        cudaEvent_t *ev = new (std::nothrow) cudaEvent_t[nchunks]();
+        if (!ev) return fail(PCPD_ERR_ALLOC, "host allocation failed");
+        for (uint32_t c = 0; c < h->n_chunk_ev; ++c) ev[c] = h->chunk_ev[c];
+        delete[] h->chunk_ev;
+        h->chunk_ev = ev;
+        for (; e == cudaSuccess && h->n_chunk_ev < nchunks; ++h->n_chunk_ev)
+            e = cudaEventCreateWithFlags(&h->chunk_ev[h->n_chunk_ev], cudaEventDisableTiming);
+        if (e != cudaSuccess) --h->n_chunk_ev;   // (the slot of the failed creation holds nothing)
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "step_from_host: copy stream / events");
+    uint64_t *stage = (uint64_t *)dev_alloc(h->mem, bytes, h->stream);
+    if (!stage) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
+    cudaStream_t copy = h->copy_stream;
+    cudaEvent_t *ev = h->chunk_ev;
+    // From here on the lattice is overwritten chunk by chunk: a failure leaves it partly new, partly swept, so the
+    // handle is marked invalid until the whole step has been queued without error (pcpd.h).
+    h->invalid = true;
     // the copies start once everything already queued on the handle's stream has finished with the lattice
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventRecord(start, h->stream);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, start, 0);
+    e = cudaEventRecord(h->copy_start, h->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, h->copy_start, 0);
     for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
         const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
         uint64_t *dst = stage + (size_t)w0 * L;   // chunk held densely as [L][nw]
@@ -539,34 +634,32 @@ int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, 
         if (e == cudaSuccess) e = cudaEventRecord(ev[c], copy);
     }
     int rc = PCPD_OK;
-    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
+    for (uint32_t c = 0; e == cudaSuccess && rc == PCPD_OK && c < nchunks; ++c) {
         const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
         e = cudaStreamWaitEvent(h->stream, ev[c], 0);
         if (e != cudaSuccess) break;
-        g_launches += launch_permute(stage + (size_t)w0 * L, h->lat + (size_t)w0 * L, L, nw, 1, 1, h->stream);
+        g_launches += launch_transpose(stage + (size_t)w0 * L, h->lat + (size_t)w0 * L, L, nw, 1, h->stream);
         SweepParams Pc = h->P;   // the chunk as a lattice of its own: columns w0 .. w0+nw-1 (columns never interact)
         Pc.lat = h->lat + (size_t)w0 * L;
         Pc.W = nw;
         Pc.word_offset = h->P.word_offset + w0;
         for (uint64_t it = 0; it < n_sweeps; ++it) {
             Pc.t = (uint32_t)(h->sweep + it);
-            g_launches += launch_sweep(Pc, h->variant, false, h->stream, &h->jit, nullptr);
+            const int nl = launch_sweep(Pc, h->variant, false, h->stream, &h->jit, nullptr);
+            if (nl < 0) { rc = cuda_fail(cudaGetLastError(), "pipelined step: sweep launch"); break; }
+            g_launches += nl;
         }
     }
-    if (e == cudaSuccess) {
+    if (e == cudaSuccess && rc == PCPD_OK) rc = check_launch("pipelined step");
+    if (e == cudaSuccess && rc == PCPD_OK) {
         h->sweep += n_sweeps;
-        rc = check_launch("pipelined step");
-        if (rc == PCPD_OK && out_counts) rc = pcpd_density(h, out_counts);
-        else if (rc == PCPD_OK) e = cudaStreamSynchronize(h->stream);
+        h->invalid = false;
+        if (out_counts) rc = pcpd_density(h, out_counts);
+        else e = cudaStreamSynchronize(h->stream);
     }
     cudaStreamSynchronize(copy);
     cudaStreamSynchronize(h->stream);
-    for (uint32_t c = 0; ev && c < nchunks; ++c)
-        if (ev[c]) cudaEventDestroy(ev[c]);
-    delete[] ev;
-    if (start) cudaEventDestroy(start);
-    if (copy) cudaStreamDestroy(copy);
-    dev_free(stage);
+    dev_free(h->mem, stage);
     if (e != cudaSuccess) return cuda_fail(e, "step_from_host");
     return rc;
 }
@@ -628,7 +721,7 @@ int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_b
 
 int pcpd_microbench(int kind, uint32_t iters, double *out_rate)
 {
-    if (kind < 0 || kind > 7 || !out_rate || iters == 0) return fail(PCPD_ERR_ARG, "microbench: bad arguments");
+    if (kind < 0 || kind >= microbench_kinds() || !out_rate || iters == 0) return fail(PCPD_ERR_ARG, "microbench: bad arguments");
     const int rc = run_microbench(kind, iters, out_rate, nullptr);
     g_launches += 4;
     if (rc != 0) return fail(rc, "microbench failed");

@@ -1,29 +1,20 @@
 // Init (C8), per-replica particle / pair counts (C9; positional popcount) and
-// canonical <-> device layout permutation.  The device layout is column-major [W][L] (Wb = 1; the
-// Wb parameter of these kernels is the general word-blocked form [W/Wb][L][Wb]).  sm_100a, HBM-bound streaming
+// canonical <-> device layout transpose.  The device layout is column-major [W][L].  sm_100a, HBM-bound streaming
 // kernels.  See DESIGN.md section 5.
 #include "pcpd_kernels.cuh"
 
 namespace pcpd {
 
-// physical index of (site i, local column w) in the word-blocked layout [W/Wb][L][Wb]
-__device__ __forceinline__ size_t phys_index(uint32_t i, uint32_t w, uint32_t L, uint32_t Wb)
-{
-    return ((size_t)(w / Wb) * L + i) * Wb + (w % Wb);
-}
-
 // ------------------------------------------------------------------ init ---
 // mode 0: all ones; 1: word(i, w) = lo64 of block (i, 0, w_global, INIT); 2: zeros.
-__global__ void init_kernel(uint64_t *lat, uint32_t L, uint32_t W, uint32_t Wb, uint32_t word_offset, int mode,
+__global__ void init_kernel(uint64_t *lat, uint32_t L, uint32_t W, uint32_t word_offset, int mode,
                             const __grid_constant__ RoundKeys rk)
 {
     const size_t total = (size_t)L * W;
     for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < total; p += (size_t)gridDim.x * blockDim.x) {
-        // p is the PHYSICAL index; recover (i, w)
-        const uint32_t wl = (uint32_t)(p % Wb);
-        const size_t r = p / Wb;
-        const uint32_t i = (uint32_t)(r % L);
-        const uint32_t w = (uint32_t)(r / L) * Wb + wl;
+        // p is the physical index w * L + i
+        const uint32_t i = (uint32_t)(p % L);
+        const uint32_t w = (uint32_t)(p / L);
         uint64_t v;
         if (mode == 0) v = ~0ull;
         else if (mode == 2) v = 0ull;
@@ -32,27 +23,28 @@ __global__ void init_kernel(uint64_t *lat, uint32_t L, uint32_t W, uint32_t Wb, 
     }
 }
 
-int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode, const RoundKeys &rk,
+int launch_init(uint64_t *lat, uint32_t L, uint32_t W, uint32_t word_offset, int mode, const RoundKeys &rk,
                 cudaStream_t stream)
 {
     const size_t total = (size_t)L * W;
     int blocks = (int)((total + 255) / 256);
     if (blocks > 148 * 16) blocks = 148 * 16;
-    init_kernel<<<blocks, 256, 0, stream>>>(lat, L, W, (uint32_t)Wb, word_offset, mode, rk);
+    init_kernel<<<blocks, 256, 0, stream>>>(lat, L, W, word_offset, mode, rk);
     return 1;
 }
 
-// --------------------------------------------------------------- permute ---
+// ------------------------------------------------------------- transpose ---
 // canonical [L][W] <-> physical column-major [W][L]: a tiled transpose through shared memory
-// (32 x 32 words, padded), both sides coalesced.  General word-blocked layouts (Wb > 1) take the
-// simple gather below; only get/set_lattice use either, never pcpd_run.
+// (32 x 32 words, padded), both sides coalesced.  Only get/set_lattice and the chunk upload of
+// pcpd_step_from_host use it, never pcpd_run.
 __global__ void __launch_bounds__(256) transpose_kernel(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst,
                                                         uint32_t rows, uint32_t cols)
 {
-    // src is rows x cols row-major, dst is cols x rows row-major
+    // src is rows x cols row-major, dst is cols x rows row-major; blockIdx.x runs over the tiles of the longer
+    // dimension (the site index: up to 2^26 tiles), blockIdx.y over those of the other (word columns)
     __shared__ uint64_t t[32][33];
-    const uint32_t tiles_c = (cols + 31) / 32;
-    const uint32_t c0 = (blockIdx.x % tiles_c) * 32, r0 = (blockIdx.x / tiles_c) * 32;
+    const bool rows_long = rows >= cols;
+    const uint32_t c0 = (rows_long ? blockIdx.y : blockIdx.x) * 32, r0 = (rows_long ? blockIdx.x : blockIdx.y) * 32;
     const uint32_t tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     for (uint32_t j = ty; j < 32; j += 8) {
         const uint32_t r = r0 + j, c = c0 + tx;
@@ -65,34 +57,13 @@ __global__ void __launch_bounds__(256) transpose_kernel(const uint64_t *__restri
     }
 }
 
-__global__ void permute_kernel(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst, uint32_t L, uint32_t W,
-                               uint32_t Wb, int to_physical)
+// to_physical: src = canonical L x W, dst = physical W x L; else the other way round
+int launch_transpose(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int to_physical, cudaStream_t stream)
 {
-    const size_t total = (size_t)L * W;
-    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < total; c += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t i = (uint32_t)(c / W), w = (uint32_t)(c % W);  // canonical index c = i*W + w
-        const size_t p = phys_index(i, w, L, Wb);
-        if (to_physical) dst[p] = src[c];
-        else dst[c] = src[p];
-    }
-}
-
-int launch_permute(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int Wb, int to_physical,
-                   cudaStream_t stream)
-{
-    if (Wb == 1) {
-        // to_physical: src = canonical L x W; else src = physical W x L
-        const uint32_t rows = to_physical ? L : W, cols = to_physical ? W : L;
-        const uint64_t tiles = (uint64_t)((cols + 31) / 32) * ((rows + 31) / 32);
-        if (tiles < (1ull << 31)) {
-            transpose_kernel<<<(uint32_t)tiles, 256, 0, stream>>>(src, dst, rows, cols);
-            return 1;
-        }
-    }
-    const size_t total = (size_t)L * W;
-    int blocks = (int)((total + 255) / 256);
-    if (blocks > 148 * 16) blocks = 148 * 16;
-    permute_kernel<<<blocks, 256, 0, stream>>>(src, dst, L, W, (uint32_t)Wb, to_physical);
+    const uint32_t rows = to_physical ? L : W, cols = to_physical ? W : L;
+    const uint32_t tr = (rows + 31) / 32, tc = (cols + 31) / 32;
+    const dim3 grid(rows >= cols ? tr : tc, rows >= cols ? tc : tr);   // grid.y <= 2048 (W <= 65535)
+    transpose_kernel<<<grid, 256, 0, stream>>>(src, dst, rows, cols);
     return 1;
 }
 
@@ -115,26 +86,31 @@ __device__ __forceinline__ void csa(uint64_t &h, uint64_t &l, uint64_t a, uint64
     l = u ^ c;
 }
 
-template <int WB, int PAIRS>
+// PAIRS = 1: pair counts, word(i) & word(next(i)); CONN = 1 (connected multispin lattice, C10): the successor of
+// (site L-1, lane j) is (site 0, lane j+1), i.e. the site-0 word rotated right by one bit.
+template <int PAIRS, int CONN>
 __global__ void __launch_bounds__(DEN_THREADS) density_kernel(const uint64_t *__restrict__ lat, uint32_t L,
                                                               uint32_t *__restrict__ counts)
 {
-    __shared__ uint32_t s_cnt[64 * WB];
-    constexpr uint32_t SPB = DEN_THREADS / WB;  // sites per block per iteration
-    const uint32_t tid = threadIdx.x, wl = tid % WB, srow = tid / WB;
+    __shared__ uint32_t s_cnt[64];
+    const uint32_t tid = threadIdx.x;
     const uint32_t wg = blockIdx.y;
-    const uint64_t *g = lat + (size_t)wg * L * WB;
-    const uint32_t s0 = blockIdx.x * (SPB * DEN_NPT);
+    const uint64_t *g = lat + (size_t)wg * L;
+    const uint32_t s0 = blockIdx.x * (DEN_THREADS * DEN_NPT);
 
-    for (uint32_t k = tid; k < 64 * WB; k += DEN_THREADS) s_cnt[k] = 0;
+    if (tid < 64) s_cnt[tid] = 0;
 
     auto load = [&](uint32_t it) -> uint64_t {
-        const uint32_t i = s0 + it * SPB + srow;
+        const uint32_t i = s0 + it * DEN_THREADS + tid;
         if (i >= L) return 0ull;
-        uint64_t v = g[(size_t)i * WB + wl];
+        uint64_t v = g[i];
         if (PAIRS) {
-            const uint32_t i1 = (i + 1 == L) ? 0u : i + 1;
-            v &= g[(size_t)i1 * WB + wl];
+            if (i + 1 == L) {
+                const uint64_t n = g[0];
+                v &= CONN ? ((n >> 1) | (n << 63)) : n;
+            } else {
+                v &= g[i + 1];
+            }
         }
         return v;
     };
@@ -165,9 +141,9 @@ __global__ void __launch_bounds__(DEN_THREADS) density_kernel(const uint64_t *__
         }
     }
 
-    // warp: add the counters of lanes with the same column (lane % WB) bit-sliced
+    // warp: add the 32 lanes' counters bit-sliced
 #pragma unroll
-    for (int off = 16; off >= WB; off >>= 1) {
+    for (int off = 16; off >= 1; off >>= 1) {
         uint64_t carry = 0;
 #pragma unroll
         for (int p = 0; p < DEN_PLANES; ++p) {
@@ -180,41 +156,31 @@ __global__ void __launch_bounds__(DEN_THREADS) density_kernel(const uint64_t *__
     }
     __syncthreads();  // s_cnt zeroed
 
-    // every lane of a column group now holds that column's warp total; lane
-    // q = lane / WB of the group expands lanes j = q, q + 32/WB, ...
-    constexpr uint32_t GROUP = 32 / WB;
-    const uint32_t q = (tid % 32) / WB;
+    // every lane now holds the warp total; lane q expands replica lanes j = q and q + 32
+    const uint32_t q = tid % 32;
 #pragma unroll
-    for (uint32_t m = 0; m < 64 / GROUP; ++m) {
-        const uint32_t j = q + m * GROUP;
+    for (uint32_t m = 0; m < 2; ++m) {
+        const uint32_t j = q + m * 32;
         uint32_t cnt = 0;
 #pragma unroll
         for (int p = 0; p < DEN_PLANES; ++p) cnt += (uint32_t)((pl[p] >> j) & 1ull) << p;
-        if (cnt) atomicAdd(&s_cnt[wl * 64 + j], cnt);
+        if (cnt) atomicAdd(&s_cnt[j], cnt);
     }
     __syncthreads();
-    for (uint32_t k = tid; k < 64 * WB; k += DEN_THREADS) {
-        const uint32_t cnt = s_cnt[k];
-        if (cnt) atomicAdd(&counts[(size_t)wg * WB * 64 + k], cnt);
+    if (tid < 64) {
+        const uint32_t cnt = s_cnt[tid];
+        if (cnt) atomicAdd(&counts[(size_t)wg * 64 + tid], cnt);
     }
 }
 
-template <int WB>
-static void launch_density_t(const uint64_t *lat, uint32_t L, uint32_t W, int pairs, uint32_t *counts,
-                             cudaStream_t stream)
-{
-    const uint32_t sites_per_block = (DEN_THREADS / WB) * DEN_NPT;
-    dim3 grid((L + sites_per_block - 1) / sites_per_block, W / WB);
-    if (pairs) density_kernel<WB, 1><<<grid, DEN_THREADS, 0, stream>>>(lat, L, counts);
-    else density_kernel<WB, 0><<<grid, DEN_THREADS, 0, stream>>>(lat, L, counts);
-}
-
-int launch_density(const uint64_t *lat, uint32_t L, uint32_t W, int Wb, int pairs, uint32_t *counts_dev,
+int launch_density(const uint64_t *lat, uint32_t L, uint32_t W, int pairs, int connected, uint32_t *counts_dev,
                    cudaStream_t stream)
 {
-    if (Wb == 4) launch_density_t<4>(lat, L, W, pairs, counts_dev, stream);
-    else if (Wb == 2) launch_density_t<2>(lat, L, W, pairs, counts_dev, stream);
-    else launch_density_t<1>(lat, L, W, pairs, counts_dev, stream);
+    const uint32_t sites_per_block = DEN_THREADS * DEN_NPT;
+    dim3 grid((L + sites_per_block - 1) / sites_per_block, W);
+    if (!pairs) density_kernel<0, 0><<<grid, DEN_THREADS, 0, stream>>>(lat, L, counts_dev);
+    else if (!connected) density_kernel<1, 0><<<grid, DEN_THREADS, 0, stream>>>(lat, L, counts_dev);
+    else density_kernel<1, 1><<<grid, DEN_THREADS, 0, stream>>>(lat, L, counts_dev);
     return 1;
 }
 

@@ -1,6 +1,6 @@
 // Hand-written sm_100a kernels of the PCPD/TCPD multispin hot path
 // (DESIGN.md sections 4-5): sweep (RNG + masks + schedule + bitwise rule), init,
-// density (positional popcount), layout permutation.
+// density (positional popcount), layout transpose.
 //
 // Citations: update rule = Alg. 1 PAPER.md:45-70 in the bitwise form of Alg. 2
 // PAPER.md:126-151 (typos fixed per DESIGN.md readings G5/G6); schedule SD2 and
@@ -41,15 +41,14 @@ __device__ __forceinline__ uint64_t lazy_mask(uint64_t rel, const Threshold th, 
 }
 
 // ---------------------------------------------------------------------------
-// GENERIC FALLBACK (schedules with more than 32 domains per tile; WB = 1 in the column-major
-// layout).  One sweep of schedule SD2(Ts, D, A) (C5).  Grid (L/Ts tiles, W/WB word
-// groups); block = n * WB threads, thread (b, w') owns domain b of word column
-// w' for the whole sweep; the tile lives in shared memory from load to store,
-// so the lattice crosses HBM exactly once in each direction per sweep.
-template <int VARIANT, int WB>
+// GENERIC FALLBACK (schedules with more than 32 domains per tile).  One sweep of schedule
+// SD2(Ts, D, A) (C5).  Grid (L/Ts tiles, W word columns); block = n threads, thread b owns
+// domain b of the block's tile column for the whole sweep; the tile column lives in shared
+// memory from load to store, so the lattice crosses HBM exactly once in each direction per sweep.
+template <int VARIANT>
 __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
 {
-    extern __shared__ __align__(16) uint64_t tile[];  // [Ts][WB]
+    extern __shared__ __align__(16) uint64_t tile[];  // [Ts]
     __shared__ uint32_t s_sigma[MAX_SUBSTEPS];
     __shared__ uint32_t s_Sigma;
 
@@ -68,28 +67,17 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
 
     // C5 step 2: tile tau covers global sites (Sigma + tau*Ts + y) mod L.
     const uint32_t start = (uint32_t)(((uint64_t)s_Sigma + (uint64_t)tau * Ts) % L);
-    uint64_t *g = P.lat + (size_t)wg * L * WB;
-    if constexpr (WB >= 2) {
-        constexpr uint32_t CPR = WB / 2;  // 16-byte chunks per site row
-        const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
-        ulonglong2 *t2 = reinterpret_cast<ulonglong2 *>(tile);
-        for (uint32_t c = tid; c < Ts * CPR; c += nthr) {
-            uint32_t i = start + c / CPR;
-            if (i >= L) i -= L;
-            t2[c] = g2[(size_t)i * CPR + c % CPR];
-        }
-    } else {
-        for (uint32_t y = tid; y < Ts; y += nthr) {
-            uint32_t i = start + y, rot = 0;
-            if (i >= L) { i -= L; rot = P.connected; }  // connected multispin lattice (C10): bit rotation past the wrap
-            const uint64_t v = g[i];
-            tile[y] = (v >> rot) | (v << ((64u - rot) & 63u));
-        }
+    uint64_t *g = P.lat + (size_t)wg * L;
+    for (uint32_t y = tid; y < Ts; y += nthr) {
+        uint32_t i = start + y, rot = 0;
+        if (i >= L) { i -= L; rot = P.connected; }  // connected multispin lattice (C10): bit rotation past the wrap
+        const uint64_t v = g[i];
+        tile[y] = (v >> rot) | (v << ((64u - rot) & 63u));
     }
     __syncthreads();
 
-    const uint32_t b = tid / WB, wl = tid % WB;
-    const uint32_t w = P.word_offset + wg * WB + wl;  // global word index (RNG key)
+    const uint32_t b = tid;
+    const uint32_t w = P.word_offset + wg;  // global word index (RNG key)
     const uint32_t slot0 = (tau * n + b) * D;
 
     for (uint32_t k = 0; k < S; ++k) {
@@ -115,13 +103,13 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
             if (rem > 0 && x >= lo) x += rem;
             uint32_t y0 = dbase + (uint32_t)x - 1;  // footprint x-1 .. x+Rr never straddles the seam
             if (y0 >= Ts) y0 -= Ts;
-            uint64_t *q = tile + (size_t)y0 * WB + wl;
+            uint64_t *q = tile + y0;
 
-            uint64_t sa = q[0], sb = q[WB], sc = q[2 * WB];
+            uint64_t sa = q[0], sb = q[1], sc = q[2];
             uint64_t se = 0, sf = 0, sg = 0;
-            if constexpr (VARIANT != 3) se = q[3 * WB];
-            if constexpr (VARIANT == 1 || VARIANT == 2) sf = q[4 * WB];
-            if constexpr (VARIANT == 2) sg = q[5 * WB];
+            if constexpr (VARIANT != 3) se = q[3];
+            if constexpr (VARIANT == 1 || VARIANT == 2) sf = q[4];
+            if constexpr (VARIANT == 2) sg = q[5];
 
             // C6 / Alg. 2, branch-free over the 64 replicas.
             const uint64_t Dm = lazy_mask<STREAM_DIFF>(sb | sc, P.thd, slot, t, w, P.rk);
@@ -145,50 +133,39 @@ __global__ void sweep_kernel(const __grid_constant__ SweepParams P)
             } else if constexpr (VARIANT == 1) {
                 se &= ~ann;
                 sf |= fis & ~Fm;
-                q[4 * WB] = sf;
+                q[4] = sf;
             } else {
                 se &= ~ann;
                 sf &= ~ann;
                 sg |= fis & ~Fm;
-                q[4 * WB] = sf;
-                q[5 * WB] = sg;
+                q[4] = sf;
+                q[5] = sg;
             }
             q[0] = sa;
-            q[WB] = nb;
-            q[2 * WB] = nc;
-            if constexpr (VARIANT != 3) q[3 * WB] = se;
+            q[1] = nb;
+            q[2] = nc;
+            if constexpr (VARIANT != 3) q[3] = se;
         }
         __syncthreads();
     }
 
     // store the tile
-    if constexpr (WB >= 2) {
-        constexpr uint32_t CPR = WB / 2;
-        ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
-        const ulonglong2 *t2 = reinterpret_cast<const ulonglong2 *>(tile);
-        for (uint32_t c = tid; c < Ts * CPR; c += nthr) {
-            uint32_t i = start + c / CPR;
-            if (i >= L) i -= L;
-            g2[(size_t)i * CPR + c % CPR] = t2[c];
-        }
-    } else {
-        for (uint32_t y = tid; y < Ts; y += nthr) {
-            uint32_t i = start + y, rot = 0;
-            if (i >= L) { i -= L; rot = P.connected; }
-            const uint64_t v = tile[y];
-            g[i] = (v << rot) | (v >> ((64u - rot) & 63u));
-        }
+    for (uint32_t y = tid; y < Ts; y += nthr) {
+        uint32_t i = start + y, rot = 0;
+        if (i >= L) { i -= L; rot = P.connected; }
+        const uint64_t v = tile[y];
+        g[i] = (v << rot) | (v >> ((64u - rot) & 63u));
     }
 }
 
-size_t sweep_smem_bytes(uint32_t Ts, int Wb) { return (size_t)Ts * Wb * 8; }
+size_t sweep_smem_bytes(uint32_t Ts) { return (size_t)Ts * 8; }
 
 template <int VARIANT>
 static int launch_sweep_t(const SweepParams &P, cudaStream_t stream)
 {
     dim3 grid(P.L / P.Ts, P.W);
     dim3 block(P.n);
-    sweep_kernel<VARIANT, 1><<<grid, block, sweep_smem_bytes(P.Ts, 1), stream>>>(P);
+    sweep_kernel<VARIANT><<<grid, block, sweep_smem_bytes(P.Ts), stream>>>(P);
     return 1;
 }
 
@@ -206,13 +183,13 @@ int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cud
 int configure_kernels()
 {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(sweep_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(sweep_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
-    if ((e = cudaFuncSetAttribute(sweep_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(sweep_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
-    if ((e = cudaFuncSetAttribute(sweep_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(sweep_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
-    if ((e = cudaFuncSetAttribute(sweep_kernel<3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(sweep_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess)
         return (int)e;
     return configure_warp_kernels();
 }

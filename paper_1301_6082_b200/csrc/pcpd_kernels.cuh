@@ -77,10 +77,11 @@ void split_teardown(SplitSlot *s);
 size_t split_mask_bytes(const SweepParams &P);
 bool split_supported(uint32_t Ts, uint32_t D);
 
-// Launchers (all asynchronous on `stream`); return the number of kernels launched.
+// Launchers (all asynchronous on `stream`); return the number of kernels launched (launch_sweep: or -1 if a stream /
+// event operation of the two-kernel path failed; launch errors themselves surface in the caller's cudaGetLastError).
 int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit,
                  SplitSlot *split);
-// warp-per-(tile, column) production kernel (sweep_warp.cu); needs the column-major layout (Wb = 1)
+// warp-per-(tile, column) production kernel (sweep_warp.cu)
 bool sweep_warp_supported(uint32_t Ts, uint32_t D);
 int sweep_warp_wpb(uint32_t Ts, uint64_t ntasks);
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split);
@@ -98,20 +99,21 @@ uint64_t jit_launch_count();
 // compile only (no device needed): returns 0 and the cubin size; used by the CPU-side build check
 int jit_compile_only(const JitSpec &js, size_t *cubin_bytes);
 int configure_warp_kernels();
-int launch_init(uint64_t *lat, uint32_t L, uint32_t W, int Wb, uint32_t word_offset, int mode,
-                const RoundKeys &rk, cudaStream_t stream);
-// counts[64*w + j] (device, uint32[64*W]) must be zero on entry; pairs != 0 counts q(i) & q(i+1).
-int launch_density(const uint64_t *lat, uint32_t L, uint32_t W, int Wb, int pairs, uint32_t *counts_dev,
+int launch_init(uint64_t *lat, uint32_t L, uint32_t W, uint32_t word_offset, int mode, const RoundKeys &rk,
+                cudaStream_t stream);
+// counts[64*w + j] (device, uint32[64*W]) must be zero on entry; pairs != 0 counts q(i) & q(next(i)), with the ring
+// closure of the connected multispin lattice (C10) when connected != 0.
+int launch_density(const uint64_t *lat, uint32_t L, uint32_t W, int pairs, int connected, uint32_t *counts_dev,
                    cudaStream_t stream);
-// canonical [L][W] <-> word-blocked [W/Wb][L][Wb]
-int launch_permute(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int Wb, int to_physical,
-                   cudaStream_t stream);
+// canonical [L][W] <-> device column-major [W][L]
+int launch_transpose(const uint64_t *src, uint64_t *dst, uint32_t L, uint32_t W, int to_physical, cudaStream_t stream);
 // Opt-in shared memory size etc.; returns cudaError_t as int.
 int configure_kernels();
-size_t sweep_smem_bytes(uint32_t Ts, int Wb);
+size_t sweep_smem_bytes(uint32_t Ts);
 
 // microbenchmarks (microbench.cu)
 int run_microbench(int kind, uint32_t iters, double *out_rate, cudaStream_t stream);
+int microbench_kinds();   // kinds 0 .. microbench_kinds() - 1 exist
 #endif  // !__CUDACC_RTC__
 
 }  // namespace pcpd

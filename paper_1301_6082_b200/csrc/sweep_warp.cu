@@ -196,21 +196,26 @@ void split_teardown(SplitSlot *s)
     s->aux = nullptr;
 }
 
-// masks of sweep t into buf[t & 1], on the auxiliary stream, once the last reader of that buffer has finished
-static void split_produce(const SweepParams &P, uint32_t t, SplitSlot *split)
+// masks of sweep t into buf[t & 1], on the auxiliary stream, once the last reader of that buffer has finished;
+// false if a stream / event operation or the launch failed (the CUDA error stays pending for the caller)
+static bool split_produce(const SweepParams &P, uint32_t t, SplitSlot *split)
 {
     const int i = (int)(t & 1u);
     SweepParams Q = P;
     Q.t = t;
     Q.mask_dev = split->buf[i];
-    if (split->freed_valid[i]) cudaStreamWaitEvent(split->aux, split->freed[i], 0);
+    split->held[i] = -1;
+    if (split->freed_valid[i] && cudaStreamWaitEvent(split->aux, split->freed[i], 0) != cudaSuccess) return false;
     const uint32_t nwarps = (Q.L / Q.Ts) * Q.W * Q.S * Q.A;
     mask_kernel<<<(nwarps + 3) / 4, 128, 0, split->aux>>>(Q);
-    cudaEventRecord(split->ready[i], split->aux);
+    if (cudaPeekAtLastError() != cudaSuccess) return false;
+    if (cudaEventRecord(split->ready[i], split->aux) != cudaSuccess) return false;
     split->held[i] = (int64_t)t;
+    return true;
 }
 
-// Small problems: two launches per sweep; the masks of sweep t + 1 are produced while sweep t is applied.
+// Small problems: two launches per sweep; the masks of sweep t + 1 are produced while sweep t is applied.  Returns the
+// number of kernels launched, or -1 if a stream / event operation failed (nothing more is launched then).
 static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t stream, SplitSlot *split)
 {
     SweepParams P = P0;
@@ -223,17 +228,21 @@ static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t s
     const int i = (int)(t & 1u);
     int launched = 1;
     if (split->held[i] != (int64_t)t) {   // not prefetched (first sweep of the handle, or the counter was set)
-        split_produce(P, t, split);
+        if (!split_produce(P, t, split)) return -1;
         ++launched;
     }
     if (t != 0xffffffffu && split->held[i ^ 1] != (int64_t)t + 1) {
-        split_produce(P, t + 1u, split);
+        if (!split_produce(P, t + 1u, split)) return -1;
         ++launched;
     }
-    cudaStreamWaitEvent(stream, split->ready[i], 0);
+    if (cudaStreamWaitEvent(stream, split->ready[i], 0) != cudaSuccess) return -1;
     P.mask_dev = split->buf[i];
     split_consumer_any(variant, P.pmask_paper ? 1 : 0, &P, stream);
-    cudaEventRecord(split->freed[i], stream);
+    if (cudaEventRecord(split->freed[i], stream) != cudaSuccess) {
+        split->freed_valid[i] = false;
+        split->held[i] = -1;   // the buffer's reader cannot be tracked: do not reuse its contents
+        return -1;
+    }
     split->freed_valid[i] = true;
     split->launches += (uint64_t)launched;
     return launched;

@@ -92,6 +92,52 @@ def test_product_does_not_import_oracle():
         "(paper_1301_6082_b200)", "")
 
 
+def test_delta_eff_on_the_papers_scaling_form(lib):
+    """pcpd_delta_eff (host-side analysis): on rho(t) = c1 t^-delta + c2 t^-2delta (eq. (2)) the
+    effective exponent is -d ln rho / d ln t = delta (c1 t^-delta + 2 c2 t^-2delta) / rho; the library's central
+    log-log difference must reproduce it (to the O(h^2) of the difference and the rounding of the counts), and a pure
+    power law exactly.  The definition is also written out in numpy and compared element by element."""
+    import numpy as np
+
+    import paper_1301_6082_b200 as pk
+
+    L, R = 1 << 22, 128
+    times = np.array([t for t in wl.record_times(10_000) if t > 0], dtype=np.uint64)
+    tt = times.astype(np.float64)
+    delta, c1, c2 = 0.2, 0.9, -0.35
+    rho_true = c1 * tt ** -delta + c2 * tt ** (-2 * delta)
+    rng = np.random.Generator(np.random.PCG64(5))
+    counts = np.round(rho_true[:, None] * L * (1 + 1e-4 * rng.standard_normal((len(tt), R)))).astype(np.uint32)
+    for m in (1, 3):
+        rho, de = pk.delta_eff(times, counts, L, half_window=m)
+        assert np.allclose(rho, counts.astype(np.float64).mean(axis=1) / L, rtol=1e-13)
+        # the definition, written out
+        ref = np.full(len(tt), np.nan)
+        for k in range(m, len(tt) - m):
+            ref[k] = -np.log(rho[k + m] / rho[k - m]) / np.log(tt[k + m] / tt[k - m])
+        assert np.array_equal(np.isnan(de), np.isnan(ref)) and np.isnan(de[:m]).all() and np.isnan(de[-m:]).all()
+        assert np.allclose(de[m:-m], ref[m:-m], rtol=1e-12)
+        # against the analytic derivative at the window's log-midpoint
+        tm = np.sqrt(tt[2 * m:] * tt[:-2 * m])
+        exact = delta * (c1 * tm ** -delta + 2 * c2 * tm ** (-2 * delta)) / (c1 * tm ** -delta + c2 * tm ** (-2 * delta))
+        sel = tt[m:-m] >= 20            # (below, the record times are integers a factor 1.1 .. 2 apart: O(h^2) is not small)
+        assert np.max(np.abs(de[m:-m][sel] - exact[sel])) < 2e-3
+    # a pure power law gives delta at every interior point
+    pure = np.round(0.7 * tt[:, None] ** -0.159 * L * np.ones((1, 4))).astype(np.uint32)
+    _, de = pk.delta_eff(times, pure, L, 2)
+    assert np.allclose(de[2:-2], 0.159, atol=2e-6)
+    # degenerate windows: t = 0, repeated times, zero density -> NaN, not an error
+    t2 = np.array([0, 1, 2, 2, 2, 4, 8], dtype=np.uint64)
+    c = np.array([[9], [8], [7], [7], [7], [0], [5]], dtype=np.uint32)
+    _, de = pk.delta_eff(t2, c, 16, 1)
+    assert np.isnan(de[[0, 1, 3, 4, 6]]).all() and np.isfinite(de[[2, 5]]).all()
+    # argument errors
+    r, dl = np.empty(7), np.empty(7)
+    assert lib.pcpd_delta_eff(t2.ctypes.data, 7, c.ctypes.data, 1, 16, 0, r.ctypes.data, dl.ctypes.data) < 0
+    assert lib.pcpd_delta_eff(t2[::-1].copy().ctypes.data, 7, c.ctypes.data, 1, 16, 1, r.ctypes.data, dl.ctypes.data) < 0
+    assert lib.pcpd_delta_eff(None, 7, c.ctypes.data, 1, 16, 1, r.ctypes.data, dl.ctypes.data) < 0
+
+
 def test_record_times():
     t = wl.record_times(10_000)
     assert t[0] == 0 and t[1] == 1 and t[-1] == 10_000 and t == sorted(set(t))

@@ -1,4 +1,4 @@
-"""Pins P0-P4, P7 of the CPU oracle (SURVEY.md 8(c) "What pins the oracle").
+"""Pins P0-P4, P7, P9-P12 of the CPU oracle (SURVEY.md 8(c) "What pins the oracle").
 
 Everything here is checked against something OTHER than the oracle itself:
 published Philox vectors, exact rational arithmetic, structural invariants of
@@ -307,6 +307,136 @@ def test_P7_run_splitting_loop_order_word_subsets(variant):
     s2 = oracle.Oracle(**kw)
     s2.set_words(w)
     assert np.array_equal(s2.get_words(), w)
+
+
+def _bits_of(words):
+    return ((words[:, :, None] >> np.arange(64, dtype=np.uint64)) & np.uint64(1)).astype(np.uint32)   # [L, W, 64]
+
+
+def test_P7_pair_counts_against_numpy_including_the_ring_closure():
+    """oracle_pair_counts = sum_i q(i) q(i+1 mod L) per replica (PAPER.md:203-208), against numpy on the packed words;
+    states built so that a dropped or wrong ring closure (site L-1 -> site 0) changes the answer."""
+    L, W = 96, 3
+    o = oracle.Oracle(L, 64 * W, 0.3, 0.1, 3, wl.PCPD, Ts=96, D=32, A=4)
+    for trial, w in enumerate([wl.random_lattice_words(L, W, 0.5, seed=11), wl.random_lattice_words(L, W, 0.8, seed=12)]):
+        w[0, :] |= np.uint64(0x00FF00FF00FF00FF)      # plenty of (L-1, 0) pairs ...
+        w[L - 1, :] |= np.uint64(0x0F0F0F0F0F0F0F0F)
+        w[1, :] &= ~np.uint64(0xFFFF)                 # ... that are not mirrored by (0, 1) pairs
+        o.set_words(w)
+        expect = _bits_of(w & np.roll(w, -1, axis=0)).sum(axis=0).ravel()
+        assert np.array_equal(o.pair_counts(), expect), trial
+        no_wrap = _bits_of(w[:-1] & w[1:]).sum(axis=0).ravel()
+        assert not np.array_equal(expect, no_wrap)   # the closure did matter in this state
+    # only the closure pair: one particle at site L-1 and one at site 0 in lane 7
+    w = np.zeros((L, W), np.uint64)
+    w[0, 1] = w[L - 1, 1] = np.uint64(1 << 7)
+    o.set_words(w)
+    pc = o.pair_counts()
+    assert pc[64 + 7] == 1 and pc.sum() == 1
+    # full lattice: L pairs per replica; empty: none
+    o.init(wl.INIT_FULL)
+    assert np.all(o.pair_counts() == L)
+    o.init(wl.INIT_EMPTY)
+    assert not o.pair_counts().any()
+
+
+def test_P7_pair_counts_on_the_connected_lattice_are_those_of_the_long_ring():
+    """C10: a word column is ONE ring of 64 L sites (strand position lane*L + site); the successor of (site L-1,
+    lane j) is (site 0, lane j+1 mod 64).  The ring is unrolled here with numpy and its adjacent pairs counted by the
+    lane of their left site."""
+    L, W = 64, 2
+    w = wl.random_lattice_words(L, W, 0.6, seed=21)
+    o = oracle.Oracle(L, 64 * W, 0.3, 0.1, 3, wl.PCPD | oracle.CONNECTED, Ts=64, D=32, A=4)
+    o.set_words(w)
+    bits = _bits_of(w)                                              # [L, W, 64]
+    for k in range(W):
+        ring = bits[:, k, :].T.reshape(-1)                          # position lane*L + site
+        pairs = ring & np.roll(ring, -1)
+        assert np.array_equal(o.pair_counts()[64 * k:64 * (k + 1)], pairs.reshape(64, L).sum(axis=1))
+    # a lone pair across the lane seam: (site L-1, lane 63) and (site 0, lane 0) are neighbours on the ring
+    w = np.zeros((L, W), np.uint64)
+    w[L - 1, 0] = np.uint64(1) << np.uint64(63)
+    w[0, 0] = np.uint64(1)
+    o.set_words(w)
+    pc = o.pair_counts()
+    assert pc[63] == 1 and pc.sum() == 1
+    i = oracle.Oracle(L, 64 * W, 0.3, 0.1, 3, wl.PCPD, Ts=64, D=32, A=4)   # independent lanes: not neighbours
+    i.set_words(w)
+    assert not i.pair_counts().any()
+
+
+# ----------------------------------------------------------------- P12 ----
+# The oracle's instrumentation (SURVEY.md 8(d) "lazy-needed count": planes / Philox blocks a lazy MSB-first evaluation
+# needs until all 64 lanes of a mask are decided) - feeds bench.py's cpu_baseline.lazy_blocks_per_attempt_word and is
+# checked against the closed form the roofline numerator uses.
+def _first_deciding_plane(U, T):
+    """Brute force from C3: lane j is decided at the first plane k (1-based count) where bit (31-k) of U_j differs from
+    that of T; planes below T's lowest set bit never matter (a lane equal to T on all planes that matter is not < T)."""
+    if T == 0 or T >= 1 << 32:
+        return 0
+    nq = max(k + 1 for k in range(32) if (T >> (31 - k)) & 1)
+    need = 0
+    for u in U:
+        first = next((k + 1 for k in range(32) if ((int(u) >> (31 - k)) & 1) != ((T >> (31 - k)) & 1)), 32)
+        need = max(need, min(first, nq))
+    return need
+
+
+@pytest.mark.parametrize("d,p", [(0.8, 0.12), (0.5, 0.152), (0.75, 2.0 ** -32), (0.0, 1.0)])
+def test_P12_stats_equal_brute_force_first_differing_plane(d, p):
+    L, D = 16, 16     # one tile = one domain, one word: slot g = sub-step * A + a runs over 0 .. 15
+    seed, word, sweeps = 0x5EED0000BEEF, 5, 3
+    o = oracle.Oracle(L, 64 * 6, d, p, seed, wl.PCPD, Ts=L, D=D, A=4, words=[word])
+    o.init(wl.INIT_BERNOULLI)
+    o.run(sweeps)
+    Td, Tp = o.thresholds()
+    exp = dict(attempt_words=0, planes_needed_D=0, planes_needed_P=0, blocks_needed_D=0, blocks_needed_P=0)
+    for t in range(sweeps):
+        for g in range(L):
+            nd = _first_deciding_plane(oracle.lane_uniforms(seed, g, t, word, oracle.STREAM_DIFF), Td)
+            npp = _first_deciding_plane(oracle.lane_uniforms(seed, g, t, word, oracle.STREAM_ANNI), Tp)
+            exp["attempt_words"] += 1
+            exp["planes_needed_D"] += nd
+            exp["planes_needed_P"] += npp
+            exp["blocks_needed_D"] += (nd + 1) // 2
+            exp["blocks_needed_P"] += (npp + 1) // 2
+    assert o.stats() == exp
+
+
+def test_P12_hand_checked_masks():
+    """Four lanes worked out by hand against T = 0b1100 << 28 (0.75): U = 0b1011... differs at plane 2, 0b1101... at
+    plane 4, 0b0... at plane 1; T has two planes that matter, so the counts cap at 2."""
+    T = 0xC0000000
+    assert _first_deciding_plane([0xB0000000], T) == 2
+    assert _first_deciding_plane([0xD0000000], T) == 2      # differs at plane 4, but planes 3.. cannot matter
+    assert _first_deciding_plane([0x00000000], T) == 1
+    assert _first_deciding_plane([0x00000000, 0xB0000000], T) == 2
+    assert _first_deciding_plane([0x12345678], 0x12345679) == 32
+    assert _first_deciding_plane([0x12345678], 0) == 0 and _first_deciding_plane([5], 1 << 32) == 0
+
+
+def test_P12_stats_reproduce_the_closed_form_of_the_roofline_numerator():
+    """A lane is undecided after k planes w.p. 2^-k, so a generic 64-lane mask needs sum_m [1 - (1 - 4^-m)^64] = 3.92
+    blocks on average (bench.py's blocks_needed_generic): the oracle's instrumentation must agree
+    within its sampling error, on cfg4's thresholds."""
+    c = wl.BY_NAME["cfg4"]
+    o = oracle.Oracle(2048, 64 * 4, c.d, c.p, c.seed, c.variant)
+    o.init(c.init)
+    o.run(2)
+    st = o.stats()
+    n = st["attempt_words"]
+    assert n == 2 * 2048 * 4
+    closed = sum(1.0 - (1.0 - 4.0 ** -m) ** 64 for m in range(16))
+    assert abs(closed - 3.92) < 0.01
+    # per-mask block count has a standard deviation of ~0.96 (SURVEY.md 8(d))
+    for key in ("blocks_needed_D", "blocks_needed_P"):
+        assert abs(st[key] / n - closed) < 5 * 0.96 / n ** 0.5, (key, st[key] / n, closed)
+    # d = 1/2: exactly one plane, one block, per mask
+    o = oracle.Oracle(2048, 64, 0.5, c.p, 1, 0)
+    o.init(0)
+    o.run(1)
+    st = o.stats()
+    assert st["planes_needed_D"] == st["blocks_needed_D"] == st["attempt_words"] == 2048
 
 
 def test_init_bernoulli_is_the_init_stream():
