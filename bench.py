@@ -248,7 +248,7 @@ def int_peak_curve(pk, sm_mhz: float) -> dict:
 
 def kernel_label(h) -> str:
     return "sweep_warp_kernel" + (" (run-time specialised on T_d, T_p: csrc/jit.cu)" if h.jit_state() == 1
-                                  else " (small-problem paths: launch_ms is per sweep over all its kernels)"
+                                  else " (column_kernel: one block per tile column, producer warps + two half-word update warps)"
                                   if h.split_launch_count() > 0 else " (built-in generic-threshold kernel)")
 
 

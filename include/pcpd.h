@@ -220,19 +220,18 @@ PCPD_API const char *pcpd_jit_message(void);
 PCPD_API uint64_t pcpd_jit_launch_count(void);
 PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t *cubin_bytes);
 
-/* ---- small problems: two kernels per sweep -----------
- * With fewer tile columns ((L / T_s) * W) than the GPU has warp slots to fill, one warp per tile column leaves
- * the machine idle and each sweep is the latency of one warp's chain of D attempts.  Such handles (at most one
- * tile column per SM) run each sweep as two launches: mask_kernel computes the state-independent part of
- * ALL attempts of the sweep in parallel (MISC block, compared prefix planes of DIFF and ANNI), then the update
- * kernel reads them and applies the attempts in order; the masks do not depend on the lattice, so those of
- * sweep t+1 are computed on an internal auxiliary stream while sweep t is applied.  Same results bit for bit.  Environment, read by
- * Handles with more tile columns than SMs but at most 512 use a one-kernel form of the same idea: one block of
- * four warps per tile column, three producer warps computing the records into a shared-memory ring, one update warp.
- * pcpd_create*: PCPD_SPLIT=0 never; PCPD_SPLIT=force the two-kernel path whenever the mask buffer stays below
- * 1 GiB, PCPD_SPLIT=block the one-block form at every size (test hooks).
- * pcpd_split_launch_count: kernels this handle has launched on those paths (two-kernel: 2 per sweep + 1; one-block
- * form: 1 per sweep; 0 = fused kernel). */
+/* ---- small and mid-size problems: one block per tile column -----------
+ * With fewer tile columns ((L / T_s) * W) than the GPU has warp slots to fill, one warp per tile column leaves the
+ * machine idle and each sweep is the latency of one warp's chain of D attempts.  Handles with at most 512 tile columns
+ * therefore run column_kernel: one block per tile column in which producer warps compute the state-independent part
+ * of every attempt (MISC block, footprint position, the complete masks Dm and Pm) into a shared-memory ring and two
+ * update warps - one per 32-bit half of the 64 replica lanes, which never interact - apply the attempts in order.
+ * Same results bit for bit.  Environment, read by pcpd_create*: PCPD_SPLIT=0 never (the fused kernel at every size);
+ * PCPD_SPLIT=column at every size; PCPD_SPLIT=force / block: two earlier forms of the same idea, kept as cross-checks
+ * for the parity tests (two kernels per sweep - mask_kernel + update kernel - whenever the mask buffer stays below
+ * 1 GiB / a four-warp producer-consumer block per tile column); PCPD_COL_NPROD = producer warps per block (tuning).
+ * pcpd_split_launch_count: kernels this handle has launched on those paths (column / block: 1 per sweep; force:
+ * 2 per sweep + 1; 0 = fused kernel). */
 PCPD_API uint64_t pcpd_split_launch_count(const pcpd_t *h);
 
 /* Number of kernels this library has launched so far in this process. */

@@ -298,25 +298,24 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         P.clp[M] = -tbit(P.thp.T32, 2 * M - 1);
     }
     {
-        // Small problems - fewer tile columns than the GPU has warp slots to fill - run each sweep as two kernels:
-        // the state-independent masks of all attempts in parallel, then the sequential update (sweep_warp.cu).
-        // PCPD_SPLIT: unset / "1" auto - at most one tile column per SM: the update kernel keeps a tile column and its
-        // 96 KB of mask records in shared memory, one block per SM, so a second wave doubles its time (measured on
-        // B200 at L = 65536: 128 columns 75 -> 38 us per sweep, 256 columns 76 -> 70 us, 512 columns 76 -> 140 us);
-        // "0" never; "force" whenever the mask buffer stays below 1 GiB.
+        // Small and mid-size problems - too few tile columns to fill the GPU with one warp each - run column_kernel
+        // (column_device.cuh): one block per tile column, producer warps computing the state-independent part of every
+        // attempt, two update warps (one per 32-bit half of the replica lanes) applying them in order.  Measured on B200
+        // at L = 65536, generic thresholds, per sweep (fused warp kernel -> column kernel): 128 columns 75 -> 18.6 us,
+        // 256: 76 -> 31 us, 512: 76 -> 57 us, 1024: 101 -> 96 us; from there on the fused kernel is as fast or faster.
+        // PCPD_SPLIT: unset / "1" auto (up to 512 tile columns); "0" never; "column" at every size (test hook);
+        // "force" / "block": the two earlier forms of the idea, kept as cross-checks for the parity tests - two kernels
+        // per sweep (mask_kernel + update kernel) whenever the mask buffer stays below 1 GiB / one producer-consumer
+        // block of four warps per tile column.
         const char *sm = getenv("PCPD_SPLIT");
-        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : !strcmp(sm, "block") ? 3 : 1;
-        // more than one tile column per SM but still too few to fill the GPU (measured on B200 up to 512: 256 columns
-        // 76 -> 47 us per sweep, 512 columns 76 -> 69 us): producer warps and the update warp in one block per tile
-        // column, records through a shared-memory ring ("block": that path at every size - test hook)
-        const uint64_t ntasks0 = (L / Ts) * W;
-        if ((mode == 3 || (mode == 1 && ntasks0 > (uint64_t)prop.multiProcessorCount && ntasks0 <= 512)) &&
-            split_block_supported(Ts, D) && !h->force_block)
-            h->split.block_mode = 1;
+        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : !strcmp(sm, "block") ? 3
+                         : !strcmp(sm, "column") ? 4 : 1;
         const uint64_t ntasks = (L / Ts) * W;
+        if ((mode == 4 || (mode == 1 && ntasks <= 512)) && column_supported(Ts, D) && !h->force_block)
+            h->split.block_mode = 2;
+        if (mode == 3 && split_block_supported(Ts, D) && !h->force_block) h->split.block_mode = 1;
         const size_t bytes = split_mask_bytes(P);
-        if (mode && mode != 3 && split_supported(Ts, D) && !h->force_block &&
-            (mode == 2 ? bytes <= (1ull << 30) : ntasks <= (uint64_t)prop.multiProcessorCount)) {
+        if (mode == 2 && split_supported(Ts, D) && !h->force_block && bytes <= (1ull << 30)) {
             h->split.buf[0] = dev_alloc(h->mem, bytes, h->stream);   // any failure here: the fused kernel is used
             h->split.buf[1] = h->split.buf[0] ? dev_alloc(h->mem, bytes, h->stream) : nullptr;
             if (!h->split.buf[1] || split_setup(&h->split) != 0) {

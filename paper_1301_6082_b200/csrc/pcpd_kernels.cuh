@@ -69,8 +69,10 @@ struct SplitSlot {
     cudaEvent_t ready[2], freed[2];
     int64_t held[2];       // -1: nothing
     bool freed_valid[2];
-    int block_mode;        // 1: SPLIT = 3 instead - producer warps and the update warp in one block per tile column
+    int block_mode;        // 1: SPLIT = 3 instead - producer warps and the update warp in one block per tile column;
+                           // 2: column_kernel - producer warps and two half-word update warps in one block per tile column
 };
+bool column_supported(uint32_t Ts, uint32_t D);
 bool split_block_supported(uint32_t Ts, uint32_t D);
 int split_setup(SplitSlot *s);     // creates the stream and events (buffers are allocated by the API layer); 0 = ok
 void split_teardown(SplitSlot *s);

@@ -4,6 +4,7 @@
 #include <cstdlib>
 
 #include "sweep_warp_device.cuh"
+#include "column_device.cuh"
 
 namespace pcpd {
 
@@ -165,6 +166,81 @@ static int launch_sweep_block4(const SweepParams &P0, int variant, cudaStream_t 
     return 1;
 }
 
+// ---- column_kernel: one block per tile column, producer warps + two update warps (column_device.cuh) ----
+static size_t column_smem_bytes(uint32_t Ts, uint32_t nprod)
+{
+    const size_t pstride = (Ts + 5u) & ~3u, slots = (size_t)COL_RING_PER_PRODUCER * nprod;
+    return ((2 * pstride * 4 + 127) & ~(size_t)127) + slots * COL_REC_BYTES + 2 * slots * 8;
+}
+
+bool column_supported(uint32_t Ts, uint32_t D) { return Ts / D <= 32 && column_smem_bytes(Ts, 2) <= 226 * 1024; }
+
+// producer warps per block (measured on B200 at L = 65536, generic thresholds): 14 (a 16-warp
+// block) while every tile column has an SM of its own - cfg2: 18.6 us per sweep with 14, 20.5 with 8, 26.6 with 4 -
+// and 8 (a 10-warp block, six of which share an SM) beyond: 256 columns 30.8 us (4: 33.2, 14: 34.9), 512 columns
+// 57.4 us (4: 63.2, 14: 67.3).
+static uint32_t column_nprod(uint32_t Ts, uint64_t ntasks)
+{
+    if (const char *e = getenv("PCPD_COL_NPROD")) {   // tuning hook
+        const int v = atoi(e);
+        if (v >= 1 && v <= 14) return (uint32_t)v;
+    }
+    uint32_t np = ntasks <= 148 ? 14u : 8u;
+    while (np > 1 && column_smem_bytes(Ts, np) > 226 * 1024) --np;
+    return np;
+}
+
+// prefix lengths of the producers (5 + 5 interleaved chains beside the MISC block for thresholds with that many blocks:
+// all 64 lanes of 32 domains need 6.4 blocks per stream on average; 1 for short thresholds, 0 for T = 0 or 2^32)
+constexpr int COL_NU_BIG = 5;
+static int col_nu_of(uint32_t nblk) { return nblk == 0 ? 0 : nblk < (uint32_t)COL_NU_BIG ? 1 : COL_NU_BIG; }
+
+template <int VARIANT, int NU_D, int NU_P>
+static int column_op(const SweepParams *P, uint32_t nprod, cudaStream_t stream)
+{
+    if (!P)
+        return (int)cudaFuncSetAttribute(column_kernel<VARIANT, NU_D, NU_P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+    column_kernel<VARIANT, NU_D, NU_P><<<(P->L / P->Ts) * P->W, (2 + nprod) * 32, column_smem_bytes(P->Ts, nprod), stream>>>(*P);
+    return 1;
+}
+
+template <int VARIANT, int NU_D>
+static int column_op_p(int nup, const SweepParams *P, uint32_t nprod, cudaStream_t stream)
+{
+    if (nup == 0) return column_op<VARIANT, NU_D, 0>(P, nprod, stream);
+    if (nup == 1) return column_op<VARIANT, NU_D, 1>(P, nprod, stream);
+    return column_op<VARIANT, NU_D, COL_NU_BIG>(P, nprod, stream);
+}
+
+template <int VARIANT>
+static int column_op_d(int nud, int nup, const SweepParams *P, uint32_t nprod, cudaStream_t stream)
+{
+    if (nud == 0) return column_op_p<VARIANT, 0>(nup, P, nprod, stream);
+    if (nud == 1) return column_op_p<VARIANT, 1>(nup, P, nprod, stream);
+    return column_op_p<VARIANT, COL_NU_BIG>(nup, P, nprod, stream);
+}
+
+static int column_any(int variant, int nud, int nup, const SweepParams *P, uint32_t nprod, cudaStream_t stream)
+{
+    switch (variant) {
+    case 0: return column_op_d<0>(nud, nup, P, nprod, stream);
+    case 1: return column_op_d<1>(nud, nup, P, nprod, stream);
+    case 2: return column_op_d<2>(nud, nup, P, nprod, stream);
+    default: return column_op_d<3>(nud, nup, P, nprod, stream);
+    }
+}
+
+static int launch_sweep_column(const SweepParams &P0, int variant, cudaStream_t stream, SplitSlot *split)
+{
+    SweepParams P = P0;
+    P.rr = variant == 3 ? 1u : 2u + (uint32_t)variant;
+    const int nud = col_nu_of((P.thd.nplanes + 1u) >> 1);
+    const int nup = P.pmask_paper ? 1 : col_nu_of((P.thp.nplanes + 1u) >> 1);   // (paper mask: ANNI block 0 only)
+    column_any(variant, nud, nup, &P, column_nprod(P.Ts, (uint64_t)(P.L / P.Ts) * P.W), stream);
+    split->launches += 1;
+    return 1;
+}
+
 size_t split_mask_bytes(const SweepParams &P) { return (size_t)(P.L / P.Ts) * P.W * P.S * P.A * 96u * sizeof(uint4); }
 
 // Small problems (SplitSlot::buf allocated by the API layer when the handle qualifies): two launches per sweep.
@@ -251,6 +327,7 @@ static int launch_sweep_split(const SweepParams &P0, int variant, cudaStream_t s
 int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t stream, JitSlot *jit, SplitSlot *split)
 {
     if (P.thr_dev) return warp_op_any(variant, wpb, PCPD_NUD_BIG, -2, &P, stream);
+    if (split && split->block_mode == 2 && !(jit && jit->mode == 2)) return launch_sweep_column(P, variant, stream, split);
     if (split && split->block_mode && !(jit && jit->mode == 2)) return launch_sweep_block4(P, variant, stream, split);
     if (split && split->buf[0] && !(jit && jit->mode == 2)) return launch_sweep_split(P, variant, stream, split);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
@@ -300,6 +377,10 @@ int configure_warp_kernels()
         for (int pmode = 0; pmode < 2; ++pmode) {
             int e = split_consumer_any(variant, pmode, nullptr, nullptr);
             if (e == 0) e = block4_any(variant, pmode, nullptr, nullptr);
+            if (e == 0 && pmode == 0)
+                for (int nud : {0, 1, COL_NU_BIG})
+                    for (int nup : {0, 1, COL_NU_BIG})
+                        if (e == 0) e = column_any(variant, nud, nup, nullptr, 0, nullptr);
             if (e != 0) return e;
         }
     return 0;

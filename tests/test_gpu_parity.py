@@ -86,9 +86,9 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
             pytest.skip("libnvrtc is not installed on this box: the built-in kernel ran (and passed the checks above)")
         assert g.jit_state() == 1, pk.jit_message()
     if expect_split is not None:  # which small-problem path ran: launches per handle on the SPLIT paths
-        # True: two-kernel path (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being
-        # launched one sweep ahead); "block": one producer/update block kernel per sweep; False: the fused kernel
-        want = 0 if not expect_split else times[-1] if expect_split == "block" else 2 * times[-1] + 1
+        # "force": two-kernel path (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being
+        # launched one sweep ahead); "column" / "block": one kernel per sweep; False: the fused kernel
+        want = 0 if not expect_split else times[-1] if expect_split in ("block", "column") else 2 * times[-1] + 1
         assert g.split_launch_count() == want
     g.close()
 
@@ -138,19 +138,20 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("split", ["auto", "0", "block"])
+@pytest.mark.parametrize("split", ["auto", "0", "force", "block"])
 @pytest.mark.parametrize("case", SMALL, ids=[f"case{i}" for i in range(len(SMALL))])
 def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
-    """Every word and count after every sweep.  split = auto: these sizes run the two-kernel small-problem path
-    (mask_kernel + update kernel) wherever the warp kernel applies (at most 32 domains per tile); split = 0: the
-    fused warp kernel (or the block kernel for more than 32 domains per tile)."""
+    """Every word and count after every sweep.  split = auto: these sizes run column_kernel (producer warps + two
+    half-word update warps in one block per tile column) wherever the warp kernel applies (at most 32 domains per tile);
+    split = 0: the fused warp kernel (or the generic block kernel for more than 32 domains per tile); force / block: the
+    two earlier small-problem forms (mask_kernel + update kernel; four-warp producer / consumer block)."""
     variant, L, R, d, p, Ts, D, A, init = case
     if split != "auto":
         monkeypatch.setenv("PCPD_SPLIT", split)
     kw = dict(L=L, n_replicas=R, d=d, p=p, seed=1000 + L + R, variant=variant)
     warp = min(Ts, L) // D <= 32
     gpu_check(pk, kw, dict(Ts=Ts, D=D, A=A), init, list(range(1, 7)),
-              expect_split=(False if split == "0" or not warp else True if split == "auto" else "block"))
+              expect_split=(False if split == "0" or not warp else "column" if split == "auto" else split))
 
 
 # cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
@@ -237,16 +238,18 @@ def test_invariants_on_gpu(pk):
         h.close()
 
 
-def test_mid_size_handle_runs_the_producer_consumer_block_kernel(pk):
-    """Between one tile column per SM and 512 tile columns the default is the one-block producer/consumer form (three
-    producer warps, one update warp, records through a shared-memory ring): sampled columns against the oracle."""
-    L, R = 65536, 64 * 8   # 32 tiles x 8 columns = 256 tile columns
-    kw = dict(L=L, n_replicas=R, d=0.1, p=0.09, seed=2, variant=0)
-    gpu_check(pk, kw, {}, 1, [1, 2, 3], words=[0, 5, 7], expect_split="block")
+def test_mid_size_handle_runs_the_column_kernel(pk):
+    """Up to 512 tile columns the default is column_kernel, with 8 producer warps per block from 149 columns on (several
+    blocks share an SM): sampled columns against the oracle at 256 and 512 tile columns; 1024 run the fused kernel."""
+    for W, words in ((8, [0, 5, 7]), (16, [3, 15])):   # 32 tiles x W columns
+        kw = dict(L=65536, n_replicas=64 * W, d=0.1, p=0.09, seed=2, variant=0)
+        gpu_check(pk, kw, {}, 1, [1, 2, 3], words=words, expect_split="column")
+    kw = dict(L=65536, n_replicas=64 * 32, d=0.1, p=0.09, seed=2, variant=0)
+    gpu_check(pk, kw, {}, 1, [1, 2], words=[31], expect_split=False)
 
 
 def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
-    """The two-kernel small-problem path produces the masks of sweep t+1 one sweep ahead on an auxiliary stream
+    """The two-kernel small-problem path (PCPD_SPLIT=force) produces the masks of sweep t+1 one sweep ahead on an auxiliary stream
     (double-buffered).  Re-initialising, and setting the sweep counter backwards, forwards or to the value already
     prefetched, must give what the fused kernel gives for the same sequence of calls."""
     def sequence(g):
@@ -259,11 +262,11 @@ def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
         g.sweep = 2 ** 32 - 2; g.run(1); out.append(g.get_lattice())   # last legal sweep: nothing to prefetch
         return out
     res = []
-    for mode in ("1", "0"):
+    for mode in ("force", "0"):
         monkeypatch.setenv("PCPD_SPLIT", mode)
         g = pk.Pcpd(4096, 192, 0.3, 0.12, 11, 0)
         res.append(sequence(g))
-        assert (g.split_launch_count() > 0) == (mode == "1")
+        assert (g.split_launch_count() > 0) == (mode == "force")
         g.close()
     for x, y in zip(*res):
         assert np.array_equal(x, y)
