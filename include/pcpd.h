@@ -157,6 +157,23 @@ PCPD_API int pcpd_pair_density(pcpd_t *h, uint32_t *out_pairs);
  * PCPD_ERR_ARG for non-ascending times, PCPD_ERR_RANGE past 2^32 - 1; on error the counter stays where it got to. */
 PCPD_API int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs);
 
+/* pcpd_run_series WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  pcpd_run_series takes its device-side record buffer from the
+ * allocator on every call; this variant keeps the records in ONE buffer of fixed size that is part of the library
+ * image - a file-scope `static __device__` array of PCPD_STATIC_SERIES_MAX_COUNTS uint32 (2 MiB; every GPU that loads
+ * the library holds it until the process exits) - and calls no cudaMalloc, cudaFree or allocating library routine.
+ * Arguments, results and errors are those of pcpd_run_series, bit for bit, plus:
+ *   PCPD_ERR_ARG if n_times * n_replicas * (number of non-NULL outputs) > PCPD_STATIC_SERIES_MAX_COUNTS;
+ *   PCPD_ERR_ARG if the handle's first sweep would still compile its run-time specialised kernel (NVRTC and the
+ *     module load allocate): run one sweep with pcpd_run first;
+ *   PCPD_ERR_DEVICE if the current device is not the one the handle was created on.
+ * The buffer is shared by ALL handles and calls on a device and keeps the last call's contents; each call clears the
+ * part it uses on its own stream before use.  Calls that overlap on the GPU (two handles on different streams, or two
+ * host threads) race on it: serialise them.  Synchronises the handle's stream before it returns. */
+#define PCPD_STATIC_SERIES_MAX_COUNTS 524288u
+PCPD_API int pcpd_run_series_static(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts,
+                                    uint32_t *out_pairs);
+
 /* Effective exponent of a density series (host-side analysis; eq. (2) and Figs 5-6:
  * "a straight line is obtained by plotting delta_eff as a function of rho"):
  *     rho[k]   = mean over the n_replicas replicas of series[k*n_replicas + r] / L

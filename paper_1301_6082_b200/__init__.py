@@ -24,6 +24,7 @@ CONNECTED = 0x200    # OR into `variant`: the paper's connected multispin lattic
 PMASK_PAPER = 0x100  # OR into `variant`: the paper's own annihilation mask (PCPD_VARIANT_PMASK_PAPER)
 INIT_FULL, INIT_BERNOULLI, INIT_EMPTY = 0, 1, 2
 DEFAULT_TS, DEFAULT_D, DEFAULT_A = 2048, 64, 4
+STATIC_SERIES_MAX_COUNTS = 524288   # PCPD_STATIC_SERIES_MAX_COUNTS of include/pcpd.h
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpcpd.so")
@@ -35,6 +36,7 @@ EXPORTS = (
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
     "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host", "pcpd_run_series", "pcpd_delta_eff",
+    "pcpd_run_series_static",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -124,6 +126,8 @@ def load_library() -> C.CDLL:
     L.pcpd_step_from_host.restype = C.c_int
     L.pcpd_split_launch_count.argtypes = [C.c_void_p]
     L.pcpd_split_launch_count.restype = C.c_uint64
+    L.pcpd_run_series_static.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
+    L.pcpd_run_series_static.restype = C.c_int
     L.pcpd_delta_eff.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
     L.pcpd_delta_eff.restype = C.c_int
     _lib = L
@@ -270,6 +274,16 @@ class Pcpd:
         pr = np.empty((len(t), self.n_replicas), dtype=np.uint32) if pairs else None
         _check(self._lib, self._lib.pcpd_run_series(self._h, t.ctypes.data, len(t), cnt.ctypes.data,
                                                     pr.ctypes.data if pairs else None))
+        return (cnt, pr) if pairs else cnt
+
+    def run_series_static(self, times, pairs=False):
+        """pcpd_run_series_static: run_series with the device-side records in the library's fixed static buffer - no
+        allocation on the device (at most STATIC_SERIES_MAX_COUNTS counts per call; one call at a time per GPU)."""
+        t = np.ascontiguousarray(times, dtype=np.uint64)
+        cnt = np.empty((len(t), self.n_replicas), dtype=np.uint32)
+        pr = np.empty((len(t), self.n_replicas), dtype=np.uint32) if pairs else None
+        _check(self._lib, self._lib.pcpd_run_series_static(self._h, t.ctypes.data, len(t), cnt.ctypes.data,
+                                                           pr.ctypes.data if pairs else None))
         return (cnt, pr) if pairs else cnt
 
     def pair_density(self, out=None) -> np.ndarray:

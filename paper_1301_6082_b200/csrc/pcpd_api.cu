@@ -105,6 +105,7 @@ struct pcpd_s {
     cudaEvent_t copy_start;
     cudaEvent_t *chunk_ev;
     uint32_t n_chunk_ev;
+    int device;        // the device that was current at create (pcpd_run_series_static checks it)
 };
 
 static void release_handle(pcpd_s *h)   // frees everything the handle owns (partially constructed handles too)
@@ -250,6 +251,7 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     h->Ts = Ts; h->D = D; h->A = A; h->word_offset = word_offset; h->sweep = 0;
     h->Td = threshold_of(d); h->Tp = threshold_of(p);
     h->invalid = false;
+    h->device = dev;
     h->connected = connected;
     h->copy_stream = nullptr; h->copy_start = nullptr; h->chunk_ev = nullptr; h->n_chunk_ev = 0;
     {
@@ -503,6 +505,86 @@ int pcpd_run_series(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t
     if (rc != PCPD_OK) return rc;
     if (e == cudaSuccess) e = es;
     if (e != cudaSuccess) return cuda_fail(e, "run_series");
+    return PCPD_OK;
+}
+
+// ---- pcpd_run_series_static: the record buffer of pcpd_run_series as a fixed array in the library image -------------
+// In host code the array's NAME is a host-side stand-in, not a device address: the kernels get the address that
+// cudaGetSymbolAddress returns, looked up once per device with that device current (g_series_ptr, guarded by g_mu).
+static __device__ __align__(256) uint32_t g_series_scratch[PCPD_STATIC_SERIES_MAX_COUNTS];
+static uint32_t *g_series_ptr[64] = {};
+
+// would the handle's next sweep compile its run-time specialised kernel (jit.cu: NVRTC + module load, which allocate)?
+// Mirrors the dispatch of launch_sweep / launch_sweep_warp.
+static bool next_sweep_would_compile(const pcpd_s *h)
+{
+    if (h->jit.state != 0 || !h->jit.mode || h->thr || h->force_block) return false;
+    if (!sweep_warp_supported(h->Ts, h->D)) return false;
+    if (h->jit.mode != 2 && (h->split.block_mode || h->split.buf[0])) return false;
+    if (h->P.thd.all || h->P.thp.all) return false;
+    return h->jit.mode == 2 || sweep_warp_wpb(h->Ts, (h->L / h->Ts) * h->W) == 7;
+}
+
+int pcpd_run_series_static(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs)
+{
+    if (!h || !times || n_times == 0 || (!out_counts && !out_pairs)) return fail(PCPD_ERR_ARG, "run_series_static: null argument");
+    for (uint64_t k = 0; k < n_times; ++k) {
+        if (times[k] < (k ? times[k - 1] : h->sweep))
+            return fail(PCPD_ERR_ARG, "run_series_static: times must ascend from the current sweep");
+        if (times[k] > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    }
+    const uint64_t nobs = (out_counts ? 1 : 0) + (out_pairs ? 1 : 0);
+    if (n_times > PCPD_STATIC_SERIES_MAX_COUNTS || n_times * h->R * nobs > PCPD_STATIC_SERIES_MAX_COUNTS)
+        return fail(PCPD_ERR_ARG,
+                    "run_series_static: %llu records x %llu replicas x %llu observable(s) exceed the maximum of %u counts "
+                    "of the static buffer: split the series or use pcpd_run_series",
+                    (unsigned long long)n_times, (unsigned long long)h->R, (unsigned long long)nobs, PCPD_STATIC_SERIES_MAX_COUNTS);
+    if (times[n_times - 1] > h->sweep && next_sweep_would_compile(h))
+        return fail(PCPD_ERR_ARG, "run_series_static: the handle's first sweep compiles its run-time specialised kernel, which "
+                                  "allocates: run one sweep with pcpd_run first");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "run_series_static: cudaGetDevice");
+    if (dev != h->device || dev < 0 || dev >= 64)
+        return fail(PCPD_ERR_DEVICE, "run_series_static: current device %d is not the handle's device %d", dev, h->device);
+    uint32_t *series = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (!g_series_ptr[dev]) {
+            uint32_t *ptr = nullptr;
+            e = cudaGetSymbolAddress((void **)&ptr, g_series_scratch);
+            if (e != cudaSuccess || !ptr) return cuda_fail(e, "run_series_static: cudaGetSymbolAddress");
+            g_series_ptr[dev] = ptr;
+        }
+        series = g_series_ptr[dev];
+    }
+    const size_t row = 4 * h->R, bytes = row * n_times * nobs;
+    // the density kernel accumulates with atomics and the buffer holds the last call's records: clear what is used
+    e = cudaMemsetAsync(series, 0, bytes, h->stream);
+    int rc = PCPD_OK;
+    for (uint64_t k = 0; e == cudaSuccess && rc == PCPD_OK && k < n_times; ++k) {
+        rc = pcpd_run(h, times[k] - h->sweep);
+        if (rc != PCPD_OK) break;
+        uint32_t *dst = series + (size_t)k * h->R * nobs;   // record k: [counts][pairs]
+        if (out_counts) g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, 0, 0, dst, h->stream);
+        if (out_pairs)
+            g_launches += launch_density(h->lat, (uint32_t)h->L, (uint32_t)h->W, 1, h->connected, dst + (out_counts ? h->R : 0),
+                                         h->stream);
+        rc = check_launch("density kernel");
+    }
+    if (e == cudaSuccess && rc == PCPD_OK) {
+        if (nobs == 1) {
+            e = cudaMemcpyAsync(out_counts ? out_counts : out_pairs, series, bytes, cudaMemcpyDeviceToHost, h->stream);
+        } else {
+            e = cudaMemcpy2DAsync(out_counts, row, series, 2 * row, row, n_times, cudaMemcpyDeviceToHost, h->stream);
+            if (e == cudaSuccess)
+                e = cudaMemcpy2DAsync(out_pairs, row, series + h->R, 2 * row, row, n_times, cudaMemcpyDeviceToHost, h->stream);
+        }
+    }
+    const cudaError_t es = cudaStreamSynchronize(h->stream);
+    if (rc != PCPD_OK) return rc;
+    if (e == cudaSuccess) e = es;
+    if (e != cudaSuccess) return cuda_fail(e, "run_series_static");
     return PCPD_OK;
 }
 
