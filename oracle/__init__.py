@@ -9,6 +9,7 @@ from __future__ import annotations
 import ctypes as C
 import os
 import subprocess
+import threading
 
 import numpy as np
 
@@ -31,60 +32,74 @@ def build(force: bool = False) -> str:
 
 
 _lib = None
+_lib_lock = threading.Lock()   # (tests run oracle handles on many threads: build and load once)
 
 
 def lib() -> C.CDLL:
     global _lib
-    if _lib is None:
-        L = C.CDLL(build())
-        u8p, u32p, u64p = C.POINTER(C.c_uint8), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
-        L.oracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
-        L.oracle_philox4x32_10.restype = None
-        L.oracle_threshold.argtypes = [C.c_double]
-        L.oracle_threshold.restype = C.c_uint64
-        L.oracle_lane_uniforms.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, u32p]
-        L.oracle_lane_uniforms.restype = None
-        L.oracle_paper_pmask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
-        L.oracle_paper_pmask.restype = None
-        L.oracle_bernoulli_mask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
-        L.oracle_bernoulli_mask.restype = None
-        L.oracle_single_attempt.argtypes = [C.c_int, C.c_uint32, u8p, C.c_uint32, C.c_int, C.c_int, C.c_int]
-        L.oracle_single_attempt.restype = None
-        L.oracle_create.argtypes = [C.c_uint64, C.c_double, C.c_double, C.c_uint64, C.c_int,
-                                    C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, u32p]
-        L.oracle_create.restype = C.c_void_p
-        L.oracle_destroy.argtypes = [C.c_void_p]
-        L.oracle_destroy.restype = None
-        L.oracle_set_reverse_order.argtypes = [C.c_void_p, C.c_int]
-        L.oracle_set_reverse_order.restype = None
-        L.oracle_sweep.argtypes = [C.c_void_p]
-        L.oracle_sweep.restype = C.c_uint32
-        L.oracle_set_sweep.argtypes = [C.c_void_p, C.c_uint32]
-        L.oracle_set_sweep.restype = None
-        L.oracle_thresholds.argtypes = [C.c_void_p, u64p, u64p]
-        L.oracle_thresholds.restype = None
-        L.oracle_set_word_probabilities.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.c_double]
-        L.oracle_set_word_probabilities.restype = C.c_int
-        L.oracle_stats.argtypes = [C.c_void_p, u64p]
-        L.oracle_stats.restype = None
-        L.oracle_init.argtypes = [C.c_void_p, C.c_int]
-        L.oracle_init.restype = C.c_int
-        L.oracle_run.argtypes = [C.c_void_p, C.c_uint64]
-        L.oracle_run.restype = C.c_int
-        L.oracle_shifts.argtypes = [C.c_void_p, C.c_uint32, u32p, u32p]
-        L.oracle_shifts.restype = None
-        L.oracle_counts.argtypes = [C.c_void_p, u32p]
-        L.oracle_counts.restype = None
-        L.oracle_pair_counts.argtypes = [C.c_void_p, u32p]
-        L.oracle_pair_counts.restype = None
-        L.oracle_get_words.argtypes = [C.c_void_p, u64p]
-        L.oracle_get_words.restype = None
-        L.oracle_set_words.argtypes = [C.c_void_p, u64p]
-        L.oracle_set_words.restype = None
-        L.oracle_literal_run.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.c_double, C.c_double, C.c_uint64,
-                                         u8p, C.c_uint32, u32p, u32p]
-        L.oracle_literal_run.restype = C.c_int
-        _lib = L
+    if _lib is not None:
+        return _lib
+    with _lib_lock:
+        if _lib is not None:
+            return _lib
+        return _load()
+
+
+def _load() -> C.CDLL:
+    global _lib
+    L = C.CDLL(build())
+    u8p, u32p, u64p = C.POINTER(C.c_uint8), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
+    L.oracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
+    L.oracle_philox4x32_10.restype = None
+    L.oracle_threshold.argtypes = [C.c_double]
+    L.oracle_threshold.restype = C.c_uint64
+    L.oracle_lane_uniforms.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, u32p]
+    L.oracle_lane_uniforms.restype = None
+    L.oracle_paper_pmask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
+    L.oracle_paper_pmask.restype = None
+    L.oracle_paper_pmask_bound.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, C.c_int, u8p]
+    L.oracle_paper_pmask_bound.restype = None
+    L.oracle_pmask_gate_threshold.argtypes = [C.c_double, C.c_int]
+    L.oracle_pmask_gate_threshold.restype = C.c_uint64
+    L.oracle_bernoulli_mask.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, u8p]
+    L.oracle_bernoulli_mask.restype = None
+    L.oracle_single_attempt.argtypes = [C.c_int, C.c_uint32, u8p, C.c_uint32, C.c_int, C.c_int, C.c_int]
+    L.oracle_single_attempt.restype = None
+    L.oracle_create.argtypes = [C.c_uint64, C.c_double, C.c_double, C.c_uint64, C.c_int,
+                                C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, u32p]
+    L.oracle_create.restype = C.c_void_p
+    L.oracle_destroy.argtypes = [C.c_void_p]
+    L.oracle_destroy.restype = None
+    L.oracle_set_reverse_order.argtypes = [C.c_void_p, C.c_int]
+    L.oracle_set_reverse_order.restype = None
+    L.oracle_sweep.argtypes = [C.c_void_p]
+    L.oracle_sweep.restype = C.c_uint32
+    L.oracle_set_sweep.argtypes = [C.c_void_p, C.c_uint32]
+    L.oracle_set_sweep.restype = None
+    L.oracle_thresholds.argtypes = [C.c_void_p, u64p, u64p]
+    L.oracle_thresholds.restype = None
+    L.oracle_set_word_probabilities.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.c_double]
+    L.oracle_set_word_probabilities.restype = C.c_int
+    L.oracle_stats.argtypes = [C.c_void_p, u64p]
+    L.oracle_stats.restype = None
+    L.oracle_init.argtypes = [C.c_void_p, C.c_int]
+    L.oracle_init.restype = C.c_int
+    L.oracle_run.argtypes = [C.c_void_p, C.c_uint64]
+    L.oracle_run.restype = C.c_int
+    L.oracle_shifts.argtypes = [C.c_void_p, C.c_uint32, u32p, u32p]
+    L.oracle_shifts.restype = None
+    L.oracle_counts.argtypes = [C.c_void_p, u32p]
+    L.oracle_counts.restype = None
+    L.oracle_pair_counts.argtypes = [C.c_void_p, u32p]
+    L.oracle_pair_counts.restype = None
+    L.oracle_get_words.argtypes = [C.c_void_p, u64p]
+    L.oracle_get_words.restype = None
+    L.oracle_set_words.argtypes = [C.c_void_p, u64p]
+    L.oracle_set_words.restype = None
+    L.oracle_literal_run.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.c_double, C.c_double, C.c_uint64,
+                                     u8p, C.c_uint32, u32p, u32p]
+    L.oracle_literal_run.restype = C.c_int
+    _lib = L
     return _lib
 
 
@@ -123,6 +138,20 @@ def paper_pmask(seed, slot, sweep, word, T4p) -> np.ndarray:
     return m
 
 
+def paper_pmask_bound(seed, slot, sweep, word, Tg, code) -> np.ndarray:
+    """The paper's annihilation mask family (oracle_paper_pmask_bound): code 0 b = 1/4, 1 b = 1/2, 2 b = 1, 3 b = 3/4."""
+    m = np.zeros(64, dtype=np.uint8)
+    lib().oracle_paper_pmask_bound(seed, slot, sweep, word, Tg, code, _p(m, C.c_uint8))
+    return m
+
+
+def pmask_gate_threshold(p: float, code: int) -> int:
+    """floor((p / b) 2^32) of the word-wide draw for bound code `code`; 2^64 - 1 if p >= b or the code is invalid."""
+    return int(lib().oracle_pmask_gate_threshold(float(p), int(code)))
+
+
+PMASK_BOUNDS = {0: 0.25, 1: 0.5, 2: 1.0, 3: 0.75}   # bound code -> b
+PMASK_BOUND_SHIFT = 10   # variant bits 10-11 hold the bound code (with PMASK_PAPER)
 CONNECTED = 0x200    # variant flag: the paper's connected multispin lattice (64 lanes = one ring of 64 L sites)
 PMASK_PAPER = 0x100  # variant flag: the paper's own annihilation mask (needs p < 1/4)
 

@@ -22,10 +22,12 @@
  *                                 isolated particles, master-equation enumeration
  *                                 of eq. (1) on rings L<=6
  *   oracle_literal_*          P4  exact E[rho] from the master equation
- *   oracle_paper_pmask        P9  the paper's own annihilation mask (Alg. 2 l.12-13):
- *                                 lane probability p, word-wide gate 4p, lanes
- *                                 independent 1/4-bits given the gate, pair
- *                                 probability p/4; P5 bias check vs literal Alg. 1
+ *   oracle_paper_pmask(_bound), oracle_pmask_gate_threshold
+ *                             P9  the paper's own annihilation masks (Alg. 2 l.12-13 and the
+ *                                 family of section 4.3, bounds b = 1/4, 1/2, 1, 3/4): lane
+ *                                 probability p, word-wide gate p/b, lanes independent b-bits
+ *                                 given the gate, pair probability p b; P5 bias check vs literal
+ *                                 Alg. 1 for every bound (the paper's "number of decorrelation bits")
  *   oracle_set_word_probabilities  P11 column k of a per-word run == column k of the uniform
  *                                 run with (d_k, p_k), bit for bit
  *   oracle_run (schedule SD2) P5  vs literal Alg. 1 (statistical), P6 exact toy
@@ -158,25 +160,51 @@ static void bernoulli_lanes(uint64_t seed, uint32_t slot, uint32_t sweep, uint32
     if (need) *need = planes_needed(U, T);
 }
 
-/* C4' - the paper's own annihilation mask (Alg. 2 lines 12-13; section 4.3,
- * PAPER.md:157-161), next-row f2 of SURVEY.md 8(f).  "aMask := RNG() and RNG()": two independent
- * raw random words give every lane an independent bit that is 1 w.p. 1/4 - here the two planes
- * `lo`, `hi` of ANNI block 0; "(RNG() < 4p) ? 1 : 0 ... gives either 1 or 0 equally for all N_r
- * bits": ONE uniform per attempt-word, shared by its 64 lanes - here x3 of the MISC
- * block (unused by C4), compared as a 32-bit integer with T4p = floor(4p * 2^32).  Lane j of the
- * mask = lo_j and hi_j and [x3 < T4p]: probability (1/4)(T4p/2^32) ~ p per lane, lanes partially
- * correlated.  Requires p < 1/4. */
-void oracle_paper_pmask(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
-                        uint64_t T4p, uint8_t mask[64])
+/* C4' - the paper's own annihilation masks (Alg. 2 lines 12-13; section 4.3,
+ * PAPER.md:157-161), next-row f2 of SURVEY.md 8(f).  The family, in the paper's words: "all N_r bits are
+ * set to 1 with probability p and all 0 otherwise ... fully correlated" (bound b = 1, no
+ * decorrelation bits); then the decorrelation step: per-lane independent bits that are 1 w.p. b, ANDed
+ * with ONE word-wide draw that is 1 w.p. p/b - Alg. 2's "aMask := RNG() and RNG()" gives b = 1/4
+ * ("(RNG() < 4p) ? 1 : 0 ... gives either 1 or 0 equally for all N_r bits"); "in the
+ * case of the bound p < 3/4, we would generate uncorrelated bits with a probability of 3/4 to be 1,
+ * and use the AND operation with correlated bits that are one with probability 4p/3";
+ * one raw word alone gives b = 1/2.  bound code: 0: b = 1/4 (lo AND hi), 1: b = 1/2 (lo), 2: b = 1
+ * (all lanes), 3: b = 3/4 (lo OR hi), lo / hi = the two planes of ANNI block 0; the word-wide uniform
+ * is x3 of the MISC block (unused by C4), compared as a 32-bit integer with Tg = floor((p/b) 2^32).
+ * Lane j of the mask = dec_j and [x3 < Tg]: probability b Tg / 2^32 ~ p per lane, two lanes both set
+ * w.p. b^2 Tg / 2^32 ~ p b.  Requires p < b. */
+static const double PMASK_BOUND[4] = { 0.25, 0.5, 1.0, 0.75 };
+
+/* Tg = floor((p / b) 2^32) for bound code c: the quotient p/b is formed in double the way the paper
+ * writes it - 4p, 2p, p, 4p/3 - then C3's floor.  UINT64_MAX for an invalid code or p >= b. */
+uint64_t oracle_pmask_gate_threshold(double p, int code)
+{
+    if (code < 0 || code > 3 || !(p >= 0.0 && p < PMASK_BOUND[code])) return UINT64_MAX;
+    double q = code == 0 ? 4.0 * p : code == 1 ? 2.0 * p : code == 2 ? p : 4.0 * p / 3.0;
+    return oracle_threshold(q);
+}
+
+void oracle_paper_pmask_bound(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
+                              uint64_t Tg, int code, uint8_t mask[64])
 {
     uint32_t a[4], misc[4];
     block(seed, slot, sweep, word, STREAM_ANNI, 0, a);
     block(seed, slot, sweep, word, STREAM_MISC, 0, misc);
     uint64_t lo = (uint64_t)a[0] | ((uint64_t)a[1] << 32);
     uint64_t hi = (uint64_t)a[2] | ((uint64_t)a[3] << 32);
-    int gate = ((uint64_t)misc[3] < T4p) ? 1 : 0;
-    for (int j = 0; j < 64; ++j)
-        mask[j] = (uint8_t)(((lo >> j) & 1u) && ((hi >> j) & 1u) && gate);
+    int gate = ((uint64_t)misc[3] < Tg) ? 1 : 0;
+    for (int j = 0; j < 64; ++j) {
+        int l = (int)((lo >> j) & 1u), h = (int)((hi >> j) & 1u);
+        int dec = code == 0 ? (l && h) : code == 1 ? l : code == 2 ? 1 : (l || h);
+        mask[j] = (uint8_t)(dec && gate);
+    }
+}
+
+/* Alg. 2's own form (b = 1/4), T4p = floor(4p 2^32). */
+void oracle_paper_pmask(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
+                        uint64_t T4p, uint8_t mask[64])
+{
+    oracle_paper_pmask_bound(seed, slot, sweep, word, T4p, 0, mask);
 }
 
 void oracle_bernoulli_mask(uint64_t seed, uint32_t slot, uint32_t sweep, uint32_t word,
@@ -269,7 +297,8 @@ void oracle_single_attempt(int variant, uint32_t L, uint8_t *q, uint32_t i,
 typedef struct oracle_t {
     uint32_t L, Ts, D, A;
     int variant;               /* 0 PCPD, 1 TCPD, 2 QCPD, 3 CPD (contact process with diffusion) */
-    int pmask_paper;           /* 1: the paper's own annihilation mask (C4', below) */
+    int pmask_paper;           /* 1: the paper's own annihilation mask (C4', above) */
+    int pmask_code;            /*    its bound code: 0 b = 1/4, 1 b = 1/2, 2 b = 1, 3 b = 3/4 */
     int connected;             /* 1: the paper's connected multispin lattice (C10, below) */
     uint64_t Td, Tp, T4p;
     uint64_t *Td_w, *Tp_w;     /* per simulated word column (index k): thresholds in force (C11) */
@@ -291,14 +320,17 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
                         uint32_t Ts, uint32_t D, uint32_t A,
                         uint32_t nwords, const uint32_t *words)
 {
-    /* variant = base | ORACLE_PMASK_PAPER (0x100): base 0 PCPD / 1 TCPD; the flag selects the
-     * paper's partially correlated annihilation mask, which needs p < 1/4. */
+    /* variant = base | ORACLE_PMASK_PAPER (0x100): base 0 PCPD / 1 TCPD / 2 QCPD / 3 CPD; the flag selects the
+     * paper's partially correlated annihilation mask; bits 10-11 (0x400, 0x800) give
+     * its bound code (0: b = 1/4 as in Alg. 2; 1: 1/2; 2: 1; 3: 3/4), which needs p < b. */
     int pmask_paper = (variant & 0x100) ? 1 : 0;
+    int pmask_code = (variant >> 10) & 3;
     /* | ORACLE_CONNECTED (0x200): the paper's connected multispin lattice, C10. */
     int connected = (variant & 0x200) ? 1 : 0;
-    variant &= ~0x300;
+    variant &= ~0xF00;
     if (variant < 0 || variant > 3) return NULL;
-    if (pmask_paper && !(p < 0.25)) return NULL;
+    if (!pmask_paper && pmask_code) return NULL;
+    if (pmask_paper && oracle_pmask_gate_threshold(p, pmask_code) == UINT64_MAX) return NULL;
     uint32_t Rr = variant == 3 ? 1u : 2u + (uint32_t)variant;   /* right reach: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD */
     if (L == 0 || L >= ((uint64_t)1 << 32) || nwords == 0) return NULL;
     if (Ts > L) Ts = (uint32_t)L;
@@ -311,8 +343,9 @@ oracle_t *oracle_create(uint64_t L, double d, double p, uint64_t seed, int varia
     if (!o) return NULL;
     o->L = (uint32_t)L; o->Ts = Ts; o->D = D; o->A = A; o->variant = variant;
     o->pmask_paper = pmask_paper;
+    o->pmask_code = pmask_code;
     o->connected = connected;
-    o->T4p = pmask_paper ? oracle_threshold(4.0 * p) : 0;   /* floor(4p * 2^32) < 2^32 since p < 1/4 */
+    o->T4p = pmask_paper ? oracle_pmask_gate_threshold(p, pmask_code) : 0;   /* floor((p/b) 2^32) < 2^32 since p < b */
     o->Td = Td; o->Tp = Tp; o->seed = seed; o->sweep = 0; o->nwords = nwords;
     o->words = (uint32_t *)malloc(sizeof(uint32_t) * nwords);
     o->Td_w = (uint64_t *)malloc(sizeof(uint64_t) * nwords);
@@ -420,7 +453,7 @@ static void attempt(oracle_t *o, uint32_t t, uint32_t Sigma, uint32_t sigma,
     uint8_t Dm[64], Pm[64];
     int needD = 0, needP = 0;
     bernoulli_lanes(o->seed, g, t, w, STREAM_DIFF, o->Td_w[k], Dm, &needD);
-    if (o->pmask_paper) { oracle_paper_pmask(o->seed, g, t, w, o->T4p, Pm); needP = 2; }
+    if (o->pmask_paper) { oracle_paper_pmask_bound(o->seed, g, t, w, o->T4p, o->pmask_code, Pm); needP = 2; }
     else bernoulli_lanes(o->seed, g, t, w, STREAM_ANNI, o->Tp_w[k], Pm, &needP);
     o->n_attempt_words += 1;
     o->planes_needed_D += (uint64_t)needD; o->planes_needed_P += (uint64_t)needP;

@@ -494,6 +494,62 @@ def test_P9_paper_pmask_probabilities():
     assert not any(oracle.paper_pmask(11, s, 3, 0, 0).any() for s in range(200))
 
 
+@pytest.mark.parametrize("code", [0, 1, 2, 3])
+def test_P9_paper_pmask_family_probabilities(code):
+    """The family of section 4.3: per-lane independent bits that are 1 w.p. b (b = 1/4: two raw words
+    ANDed; 1/2: one raw word; 1: none, "all N_r bits are set to 1 with probability p and all 0 otherwise"; 3/4: two raw
+    words ORed) ANDed with ONE word-wide draw that is 1 w.p. p/b.  Pinned to what those sentences fix: lane probability p;
+    gate probability p/b; given the gate the lanes are independent b-bits; two lanes are both set w.p. p b - p for
+    b = 1 (fully correlated), falling to p/4 with two decorrelation bits."""
+    b = oracle.PMASK_BOUNDS[code]
+    p = 0.12
+    Tg = oracle.pmask_gate_threshold(p, code)
+    from fractions import Fraction
+    q = {0: 4.0 * p, 1: 2.0 * p, 2: p, 3: 4.0 * p / 3.0}[code]           # the quotient as the paper writes it
+    assert Tg == (Fraction(q) * (1 << 32)).__floor__()
+    n = 40000
+    masks = np.array([oracle.paper_pmask_bound(11, s, 3, s % 7, Tg, code) for s in range(n)], dtype=np.float64)   # [n, 64]
+    gate = masks.any(axis=1)
+    per_word = masks.mean(axis=1)                     # words are the independent samples (lanes share the draw)
+    assert abs(per_word.mean() - p) < 4 * per_word.std(ddof=1) / n ** 0.5
+    assert abs(gate.mean() - p / b) < 4 * (p / b * (1 - p / b) / n) ** 0.5 + 1e-7   # (+ all-zero words: (1-b)^64)
+    g = masks[gate]
+    if b < 1:
+        assert abs(g.mean() - b) < 4 * (b * (1 - b) / g.size) ** 0.5
+        c = np.corrcoef(g[:, :8].T)
+        assert np.all(np.abs(c - np.eye(8)) < 5 / len(g) ** 0.5)
+    else:
+        assert np.all(g == 1)                         # no decorrelation: the whole word at once
+    both = (masks[:, 0] * masks[:, 1]).mean()
+    assert abs(both - p * b) < 4 * (p * b / n) ** 0.5
+    if code == 0:                                     # Alg. 2's own form is the b = 1/4 member
+        for s_ in range(50):
+            assert np.array_equal(oracle.paper_pmask(11, s_, 3, 2, Tg), oracle.paper_pmask_bound(11, s_, 3, 2, Tg, 0))
+    # p must lie below the bound
+    assert oracle.pmask_gate_threshold(b, code) == (1 << 64) - 1
+    assert oracle.pmask_gate_threshold(np.nextafter(b, 0), code) < (1 << 32)
+    with pytest.raises(ValueError):
+        oracle.Oracle(128, 64, 0.5, b, 1, oracle.PMASK_PAPER | (code << oracle.PMASK_BOUND_SHIFT), Ts=64, D=16, A=4)
+    with pytest.raises(ValueError):
+        oracle.Oracle(128, 64, 0.5, 0.1, 1, code << oracle.PMASK_BOUND_SHIFT if code else 0x1000, Ts=64, D=16, A=4)   # bound bits without the flag
+
+
+def test_P9_fully_correlated_mask_empties_whole_words_in_a_run():
+    """b = 1 wired into the run: with d = 0 and a full lattice an annihilation removes the pair in ALL 64 replicas of the
+    word at once ("the bits are fully correlated"), so after one sweep there are sites that are empty in
+    every replica (where no later fission - whose side is still drawn per lane - refilled them); with b = 1/4, 1/2 or 3/4
+    the lanes annihilate independently given the gate and 64 simultaneous holes do not occur."""
+    kw = dict(L=256, n_replicas=64, d=0.0, p=0.2, seed=5, Ts=64, D=16, A=16)
+    empty_words = {}
+    for code in range(4):
+        o = oracle.Oracle(variant=oracle.PMASK_PAPER | (code << oracle.PMASK_BOUND_SHIFT), **kw)
+        o.init(wl.INIT_FULL)
+        o.run(1)
+        empty_words[code] = int((o.get_words()[:, 0] == 0).sum())
+        assert o.counts().max() < 256          # something was annihilated in every replica's ring
+    assert empty_words[2] > 0 and empty_words[0] == empty_words[1] == empty_words[3] == 0, empty_words
+
+
 def test_P9_paper_pmask_mode_in_run():
     """The run uses exactly that mask: a full lattice with d = 0 (no diffusion) loses particles
     only in words whose word-wide draw fired, and p >= 1/4 is rejected."""
