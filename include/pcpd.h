@@ -68,6 +68,16 @@ enum pcpd_variant { PCPD_VARIANT_PCPD = 0, PCPD_VARIANT_TCPD = 1, PCPD_VARIANT_Q
  * Costs 3 Philox blocks per attempt-word when d is a short dyadic (d = 1/2, 1/4, 3/4: the
  * paper's AND/OR recipe for d, is what C3 reduces to for such d). */
 #define PCPD_VARIANT_PMASK_PAPER 0x100
+/* With PCPD_VARIANT_PMASK_PAPER: the other members of the paper's mask family (section 4.3): per-lane
+ * independent "decorrelation" bits that are 1 w.p. b, ANDed with the ONE word-wide draw, now 1 w.p. p/b (compared as
+ * floor((p/b) * 2^32) with p/b formed as 4p, 2p, p, 4p/3).  Default b = 1/4 (Alg. 2: two raw words ANDed);
+ * _BOUND_HALF: b = 1/2 (one raw word, plane lo of ANNI block 0); _BOUND_ONE: b = 1, no decorrelation - "all N_r bits
+ * are set to 1 with probability p and all 0 otherwise", fully correlated lanes; _BOUND_3_4: b = 3/4 (two
+ * raw words ORed; "correlated bits that are one with probability 4p/3").  Requires p < b; the bound bits
+ * without PCPD_VARIANT_PMASK_PAPER are an error.  This is the paper's "number of decorrelation bits" knob. */
+#define PCPD_VARIANT_PMASK_BOUND_HALF 0x400
+#define PCPD_VARIANT_PMASK_BOUND_ONE 0x800
+#define PCPD_VARIANT_PMASK_BOUND_3_4 0xC00
 /* Flag to OR into `variant`: the PAPER's CONNECTED multispin lattice instead of
  * 64 independent replicas per word: the 64 bit-lanes of a word column are 64 consecutive segments of
  * ONE periodic lattice of 64*L sites (strand position lane*L + site); the successor of (site L-1,

@@ -22,6 +22,8 @@ from .shard import gather_counts, max_over_ranks, shard_words  # noqa: F401
 PCPD, TCPD, QCPD, CPD = 0, 1, 2, 3
 CONNECTED = 0x200    # OR into `variant`: the paper's connected multispin lattice (PCPD_VARIANT_CONNECTED)
 PMASK_PAPER = 0x100  # OR into `variant`: the paper's own annihilation mask (PCPD_VARIANT_PMASK_PAPER)
+# with PMASK_PAPER: decorrelation bound b of the paper's mask family (default 1/4) - PCPD_VARIANT_PMASK_BOUND_*
+PMASK_BOUND_HALF, PMASK_BOUND_ONE, PMASK_BOUND_3_4 = 0x400, 0x800, 0xC00
 INIT_FULL, INIT_BERNOULLI, INIT_EMPTY = 0, 1, 2
 DEFAULT_TS, DEFAULT_D, DEFAULT_A = 2048, 64, 4
 STATIC_SERIES_MAX_COUNTS = 524288   # PCPD_STATIC_SERIES_MAX_COUNTS of include/pcpd.h

@@ -87,12 +87,13 @@ __device__ __forceinline__ void produce_column_record(const SweepParams &P, cons
         plt.hi += pund.hi * cl;
         if (P.thp.all) plt.lo = plt.hi = ~0u;
     } else if constexpr (NU_P >= 1) {
-        // the paper's own annihilation mask (Alg. 2 lines 12-13): an independent 1/4-bit per
-        // lane (the two planes of ANNI block 0 ANDed) gated by ONE word-wide draw that is 1 w.p. 4p (x3 of the MISC block)
+        // the paper's own annihilation mask (Alg. 2 lines 12-13): an independent b-bit per
+        // lane (b = 1/4: the two planes of ANNI block 0 ANDed; pmask_dec) gated by ONE word-wide draw that is 1 w.p. p/b
+        // (x3 of the MISC block)
         const U4 &pb = blks[1 + NU_D];
         const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-        plt.lo = pb.x0 & pb.x2 & gate;
-        plt.hi = pb.x1 & pb.x3 & gate;
+        plt.lo = pmask_dec(pb.x0, pb.x2, P.pmask_code) & gate;
+        plt.hi = pmask_dec(pb.x1, pb.x3, P.pmask_code) & gate;
     }
     const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
     uint4 *rec = reinterpret_cast<uint4 *>(slot);

@@ -150,7 +150,12 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
 {
     const int pmask_paper = (variant & PCPD_VARIANT_PMASK_PAPER) ? 1 : 0;
     const int connected = (variant & PCPD_VARIANT_CONNECTED) ? 1 : 0;
-    variant &= ~(PCPD_VARIANT_PMASK_PAPER | PCPD_VARIANT_CONNECTED);
+    const int pmask_code = (variant & PCPD_VARIANT_PMASK_BOUND_3_4) >> 10;   // 0: b = 1/4, 1: 1/2, 2: 1, 3: 3/4
+    variant &= ~(PCPD_VARIANT_PMASK_PAPER | PCPD_VARIANT_CONNECTED | PCPD_VARIANT_PMASK_BOUND_3_4);
+    if (pmask_code && !pmask_paper) {
+        fail(PCPD_ERR_ARG, "the PCPD_VARIANT_PMASK_BOUND_* bits need PCPD_VARIANT_PMASK_PAPER");
+        return nullptr;
+    }
     if (variant != PCPD_VARIANT_PCPD && variant != PCPD_VARIANT_TCPD && variant != PCPD_VARIANT_QCPD &&
         variant != PCPD_VARIANT_CPD) {
         fail(PCPD_ERR_ARG, "unknown variant %d", variant);
@@ -166,8 +171,9 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         fail(PCPD_ERR_ARG, "d and p must lie in [0,1]");
         return nullptr;
     }
-    if (pmask_paper && !(p < 0.25)) {
-        fail(PCPD_ERR_ARG, "the paper's annihilation mask needs p < 1/4");
+    static const double kBound[4] = {0.25, 0.5, 1.0, 0.75};
+    if (pmask_paper && !(p < kBound[pmask_code])) {
+        fail(PCPD_ERR_ARG, "the paper's annihilation mask needs p < b = %g (its decorrelation bound; default 1/4)", kBound[pmask_code]);
         return nullptr;
     }
     if (L == 0 || L > (1ull << 31) || word_offset + W >= (1ull << 32)) {
@@ -285,7 +291,10 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
     P.rk = make_round_keys(seed);
     P.connected = (uint32_t)connected;
     P.pmask_paper = (uint32_t)pmask_paper;
-    P.T4p = pmask_paper ? (uint32_t)threshold_of(4.0 * p) : 0u;   // < 2^32 because p < 1/4
+    // gate threshold floor((p/b) * 2^32) with p/b formed as the paper writes it: 4p, 2p, p, 4p/3 (< 2^32 because p < b)
+    const double gate_q = pmask_code == 0 ? 4.0 * p : pmask_code == 1 ? 2.0 * p : pmask_code == 2 ? p : 4.0 * p / 3.0;
+    P.T4p = pmask_paper ? (uint32_t)threshold_of(gate_q) : 0u;
+    P.pmask_code = (uint32_t)pmask_code;
     for (int k = 0; k < 32; ++k) {
         P.tdm[k] = ((P.thd.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;
         P.tpm[k] = ((P.thp.T32 >> (31 - k)) & 1u) ? 0xffffffffu : 0u;

@@ -26,7 +26,7 @@ struct SweepParams {
     uint32_t Ts, D, A, S, n;  // n = Ts / D domains per tile, S = D / A sub-steps
     uint32_t word_offset;     // global index of local column 0
     uint32_t t;               // sweep index
-    uint32_t T4p;             // paper annihilation mask: floor(4p * 2^32) (pmask_paper != 0), else 0
+    uint32_t T4p;             // paper annihilation mask: gate threshold floor((p/b) * 2^32) (pmask_paper != 0), else 0
     Threshold thd, thp;
     RoundKeys rk;
     // T's bit for plane k (bit 31-k) as an all-ones / all-zeros 32-lane mask, precomputed on the
@@ -47,6 +47,8 @@ struct SweepParams {
     void *mask_dev;
     uint32_t split_nud, split_nup;
     uint32_t rr;              // right reach of the variant's footprint: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
+    uint32_t pmask_code;      // paper annihilation mask: decorrelation bound b - 0: 1/4 (lo & hi), 1: 1/2 (lo), 2: 1 (all
+                              // lanes), 3: 3/4 (lo | hi), lo / hi = the planes of ANNI block 0
 };
 
 #ifndef __CUDACC_RTC__

@@ -176,6 +176,14 @@ __device__ __forceinline__ void cmp_block_sum(Mask2 &lt, Mask2 &und, const U4 &b
     cmp2h_sum(lt.hi, und.hi, blk.x1, blk.x3, tb0, tb1, s0, s1);
 }
 
+// The paper's annihilation-mask family (section 4.3): the per-lane "decorrelation" bits of one 32-lane
+// half from the two planes p0, p1 of ANNI block 0 - code 0: b = 1/4 (AND, Alg. 2 line 12), 1: 1/2 (one raw word), 2: 1
+// (none: fully correlated lanes), 3: 3/4 (OR).  The word-wide gate [x3 < floor((p/b) 2^32)] is applied by the caller.
+__device__ __forceinline__ uint32_t pmask_dec(uint32_t p0, uint32_t p1, uint32_t code)
+{
+    return code == 0u ? (p0 & p1) : code == 1u ? p0 : code == 2u ? ~0u : (p0 | p1);
+}
+
 // ---- TMA bulk copy + mbarrier (SPLIT consumer: the task's mask records are staged through shared memory) ----
 constexpr uint32_t MASK_REC_BYTES = 96u * 16u;  // one attempt: three rows of 32 uint4
 constexpr uint32_t MASK_MAX_CHUNKS = 256u;      // one bulk copy / mbarrier per sub-step (S <= MAX_SUBSTEPS = 256)
@@ -321,8 +329,8 @@ __device__ __forceinline__ void produce_record(const SweepParams &P, uint32_t ta
     } else {
         const U4 pb = philox_block(STREAM_ANNI, ps, pw, rk);
         const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-        plt.lo = pb.x0 & pb.x2 & gate;
-        plt.hi = pb.x1 & pb.x3 & gate;
+        plt.lo = pmask_dec(pb.x0, pb.x2, P.pmask_code) & gate;
+        plt.hi = pmask_dec(pb.x1, pb.x3, P.pmask_code) & gate;
     }
     const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
     rec[0] = make_uint4(misc.x0, misc.x1, y0, misc.x3);
@@ -672,12 +680,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 plt.hi += pund.hi * cl;
             } else {
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
-                // an independent 1/4-bit per lane (the two planes of ANNI block 0 ANDed) gated by ONE
-                // word-wide draw that is 1 w.p. 4p (x3 of the MISC block against floor(4p * 2^32)).
+                // an independent b-bit per lane (b = 1/4: the two planes of ANNI block 0 ANDed; pmask_dec) gated by
+                // ONE word-wide draw that is 1 w.p. p/b (x3 of the MISC block against floor((p/b) * 2^32)).
                 if constexpr (SPLIT < 2) {  // (SPLIT consumers: the producer has done this)
                     const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-                    plt.lo = pblk[0].x0 & pblk[0].x2 & gate;
-                    plt.hi = pblk[0].x1 & pblk[0].x3 & gate;
+                    plt.lo = pmask_dec(pblk[0].x0, pblk[0].x2, P.pmask_code) & gate;
+                    plt.hi = pmask_dec(pblk[0].x1, pblk[0].x3, P.pmask_code) & gate;
                 }
             }
             const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);

@@ -135,6 +135,9 @@ SMALL = [
     (0x200, 1024, 64, 0.5, 0.15, 2048, 64, 4, 0),    # same, single tile = whole ring (T_s clamped to L)
     (0x300, 147, 64, 0.37, 0.21, 49, 7, 1, 1),       # same + paper mask, odd L and T_s (64-bit tile copy path)
     (0x201, 1152, 128, 0.2, 0.3, 576, 9, 3, 1),      # same on TCPD through the block kernel (n = 64)
+    (0x500, 4096, 256, 0.75, 0.4, 2048, 64, 4, 0),   # the paper's mask family: bound b = 1/2 (one raw word), p < 1/2
+    (0x900, 2048, 192, 0.3, 0.6, 512, 64, 8, 1),     # b = 1: no decorrelation bits, fully correlated lanes
+    (0xD01, 4096, 128, 0.5, 0.7, 2048, 64, 4, 0),    # b = 3/4 (two raw words ORed, gate 4p/3) on TCPD
 ]
 
 
@@ -155,7 +158,7 @@ def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
 
 
 # cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
-JIT_CASES = [0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12, 14, 16, 17, 18, 19, 20, 22, 23, 25, 26, 27, 29]
+JIT_CASES = [0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12, 14, 16, 17, 18, 19, 20, 22, 23, 25, 26, 27, 29, 31, 32, 33]
 
 
 @pytest.mark.parametrize("idx", JIT_CASES, ids=[f"case{i}" for i in JIT_CASES])
@@ -436,6 +439,10 @@ def test_error_behaviour_of_the_boundary(pk):
         dict(L=4096, n_replicas=64, d=0.5, p=float("nan")),
         dict(L=4096, n_replicas=64, d=0.5, p=0.1, variant=7),  # unknown variant
         dict(L=4096, n_replicas=64, d=0.5, p=0.25, variant=pk.PMASK_PAPER),   # paper mask needs p < 1/4
+        dict(L=4096, n_replicas=64, d=0.5, p=0.5, variant=pk.PMASK_PAPER | pk.PMASK_BOUND_HALF),   # ... p < b in general
+        dict(L=4096, n_replicas=64, d=0.5, p=0.75, variant=pk.PMASK_PAPER | pk.PMASK_BOUND_3_4),
+        dict(L=4096, n_replicas=64, d=0.5, p=1.0, variant=pk.PMASK_PAPER | pk.PMASK_BOUND_ONE),
+        dict(L=4096, n_replicas=64, d=0.5, p=0.1, variant=pk.PMASK_BOUND_HALF),   # bound bits without the mask flag
         dict(L=5120, n_replicas=64, d=0.5, p=0.1),             # L % T_s != 0 (T_s = 2048 not clamped: L > T_s)
         dict(L=4096, n_replicas=64, d=0.5, p=0.1, Ts=2048, D=64, A=5),   # A does not divide D
         dict(L=4096, n_replicas=64, d=0.5, p=0.1, Ts=2048, D=6, A=2),    # D < 2*Rr + 3

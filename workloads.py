@@ -22,6 +22,7 @@ import numpy as np
 PCPD = 0  # AA0/0AA->AAA, AA->00, A0<->0A   (eq. (1))
 CONNECTED = 0x200    # variant flag: the paper's connected multispin lattice
 PMASK_PAPER = 0x100  # variant flag: the paper's own partially correlated annihilation mask
+PMASK_BOUND_HALF, PMASK_BOUND_ONE, PMASK_BOUND_3_4 = 0x400, 0x800, 0xC00   # with PMASK_PAPER: its decorrelation bound b
 TCPD = 1  # AAA0/0AAA->AAAA, AAA->000, A0<->0A (BASELINE.json config 5)
 
 QCPD = 2  # AAAA0/0AAAA->AAAAA, AAAA->0000, A0<->0A (PAPER.md:21 names it; rule by analogy with Alg. 1)
