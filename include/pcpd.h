@@ -254,11 +254,8 @@ PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t
  * of every attempt (MISC block, footprint position, the complete masks Dm and Pm) into a shared-memory ring and two
  * update warps - one per 32-bit half of the 64 replica lanes, which never interact - apply the attempts in order.
  * Same results bit for bit.  Environment, read by pcpd_create*: PCPD_SPLIT=0 never (the fused kernel at every size);
- * PCPD_SPLIT=column at every size; PCPD_SPLIT=force / block: two earlier forms of the same idea, kept as cross-checks
- * for the parity tests (two kernels per sweep - mask_kernel + update kernel - whenever the mask buffer stays below
- * 1 GiB / a four-warp producer-consumer block per tile column); PCPD_COL_NPROD = producer warps per block (tuning).
- * pcpd_split_launch_count: kernels this handle has launched on those paths (column / block: 1 per sweep; force:
- * 2 per sweep + 1; 0 = fused kernel). */
+ * PCPD_SPLIT=column at every size (test hook); PCPD_COL_NPROD = producer warps per block (tuning).
+ * pcpd_split_launch_count: column_kernel launches of this handle (1 per sweep; 0 = fused kernel). */
 PCPD_API uint64_t pcpd_split_launch_count(const pcpd_t *h);
 
 /* Number of kernels this library has launched so far in this process. */

@@ -336,7 +336,7 @@ class Pcpd:
         _check(self._lib, self._lib.pcpd_set_sweep(self._h, t))
 
     def split_launch_count(self) -> int:
-        """Kernels launched on the two-kernel small-problem path (2 per sweep; 0: fused kernel)."""
+        """column_kernel launches of this handle (small / mid-size path: 1 per sweep; 0: fused kernel)."""
         return int(self._lib.pcpd_split_launch_count(self._h))
 
     def jit_state(self) -> int:

@@ -99,7 +99,7 @@ struct pcpd_s {
     cudaStream_t stream;
     SweepParams P;
     JitSlot jit;       // threshold-specialised sweep kernel (jit.cu); mode from env PCPD_JIT at create
-    SplitSlot split;   // small problems: mask buffer of the two-kernel sweep (sweep_warp.cu); env PCPD_SPLIT
+    SplitSlot split;   // small / mid-size problems: column_kernel (sweep_warp.cu); env PCPD_SPLIT
     // pcpd_step_from_host: copy stream and events, created on first use and kept for the life of the handle
     cudaStream_t copy_stream;
     cudaEvent_t copy_start;
@@ -110,7 +110,6 @@ struct pcpd_s {
 
 static void release_handle(pcpd_s *h)   // frees everything the handle owns (partially constructed handles too)
 {
-    split_teardown(&h->split);
     if (h->copy_stream) {
         cudaStreamSynchronize(h->copy_stream);
         cudaStreamDestroy(h->copy_stream);
@@ -120,8 +119,6 @@ static void release_handle(pcpd_s *h)   // frees everything the handle owns (par
         if (h->chunk_ev[c]) cudaEventDestroy(h->chunk_ev[c]);
     delete[] h->chunk_ev;
     dev_free(h->mem, h->thr);
-    dev_free(h->mem, h->split.buf[0]);
-    dev_free(h->mem, h->split.buf[1]);
     dev_free(h->mem, h->lat);
     dev_free(h->mem, h->counts);
     delete h;
@@ -314,29 +311,11 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         // attempt, two update warps (one per 32-bit half of the replica lanes) applying them in order.  Measured on B200
         // at L = 65536, generic thresholds, per sweep (fused warp kernel -> column kernel): 128 columns 75 -> 18.6 us,
         // 256: 76 -> 31 us, 512: 76 -> 57 us, 1024: 101 -> 96 us; from there on the fused kernel is as fast or faster.
-        // PCPD_SPLIT: unset / "1" auto (up to 512 tile columns); "0" never; "column" at every size (test hook);
-        // "force" / "block": the two earlier forms of the idea, kept as cross-checks for the parity tests - two kernels
-        // per sweep (mask_kernel + update kernel) whenever the mask buffer stays below 1 GiB / one producer-consumer
-        // block of four warps per tile column.
+        // PCPD_SPLIT: unset / "1" auto (up to 512 tile columns); "0" never; "column" at every size (test hook).
         const char *sm = getenv("PCPD_SPLIT");
-        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "force") ? 2 : !strcmp(sm, "block") ? 3
-                         : !strcmp(sm, "column") ? 4 : 1;
+        const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "column") ? 2 : 1;
         const uint64_t ntasks = (L / Ts) * W;
-        if ((mode == 4 || (mode == 1 && ntasks <= 512)) && column_supported(Ts, D) && !h->force_block)
-            h->split.block_mode = 2;
-        if (mode == 3 && split_block_supported(Ts, D) && !h->force_block) h->split.block_mode = 1;
-        const size_t bytes = split_mask_bytes(P);
-        if (mode == 2 && split_supported(Ts, D) && !h->force_block && bytes <= (1ull << 30)) {
-            h->split.buf[0] = dev_alloc(h->mem, bytes, h->stream);   // any failure here: the fused kernel is used
-            h->split.buf[1] = h->split.buf[0] ? dev_alloc(h->mem, bytes, h->stream) : nullptr;
-            if (!h->split.buf[1] || split_setup(&h->split) != 0) {
-                cudaGetLastError();
-                split_teardown(&h->split);
-                dev_free(h->mem, h->split.buf[0]);
-                dev_free(h->mem, h->split.buf[1]);
-                h->split.buf[0] = h->split.buf[1] = nullptr;
-            }
-        }
+        if ((mode == 2 || (mode == 1 && ntasks <= 512)) && column_supported(Ts, D) && !h->force_block) h->split.column_mode = 1;
     }
     g_err[0] = 0;
     return h;
@@ -401,11 +380,7 @@ pcpd_t *pcpd_create_scan(uint64_t L, uint64_t n_replicas, const double *d_w, con
     }
     h->P.thr_dev = h->thr;
     h->force_block = false;
-    h->split.block_mode = 0;
-    split_teardown(&h->split);   // per-word thresholds run the fused kernel
-    dev_free(h->mem, h->split.buf[0]);
-    dev_free(h->mem, h->split.buf[1]);
-    h->split.buf[0] = h->split.buf[1] = nullptr;
+    h->split.column_mode = 0;   // per-word thresholds run the fused kernel
     return h;
 }
 
@@ -450,9 +425,7 @@ int pcpd_run(pcpd_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     for (uint64_t it = 0; it < n_sweeps; ++it) {
         h->P.t = (uint32_t)h->sweep;
-        const int nl = launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit, &h->split);
-        if (nl < 0) return cuda_fail(cudaGetLastError(), "sweep launch (stream / event operation of the two-kernel path)");
-        g_launches += nl;
+        g_launches += launch_sweep(h->P, h->variant, h->force_block, h->stream, &h->jit, &h->split);
         h->sweep += 1;
     }
     return check_launch("sweep kernel");
@@ -529,7 +502,7 @@ static bool next_sweep_would_compile(const pcpd_s *h)
 {
     if (h->jit.state != 0 || !h->jit.mode || h->thr || h->force_block) return false;
     if (!sweep_warp_supported(h->Ts, h->D)) return false;
-    if (h->jit.mode != 2 && (h->split.block_mode || h->split.buf[0])) return false;
+    if (h->jit.mode != 2 && h->split.column_mode) return false;
     if (h->P.thd.all || h->P.thp.all) return false;
     return h->jit.mode == 2 || sweep_warp_wpb(h->Ts, (h->L / h->Ts) * h->W) == 7;
 }
@@ -735,9 +708,7 @@ int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, 
         Pc.word_offset = h->P.word_offset + w0;
         for (uint64_t it = 0; it < n_sweeps; ++it) {
             Pc.t = (uint32_t)(h->sweep + it);
-            const int nl = launch_sweep(Pc, h->variant, false, h->stream, &h->jit, nullptr);
-            if (nl < 0) { rc = cuda_fail(cudaGetLastError(), "pipelined step: sweep launch"); break; }
-            g_launches += nl;
+            g_launches += launch_sweep(Pc, h->variant, false, h->stream, &h->jit, nullptr);
         }
     }
     if (e == cudaSuccess && rc == PCPD_OK) rc = check_launch("pipelined step");

@@ -42,10 +42,6 @@ struct SweepParams {
     const uint32_t *thr_dev;
     uint32_t connected;       // 1: connected multispin lattice: words of tile sites past the ring wrap are bit-rotated (C10)
     uint32_t pmask_paper;     // 1: Pm = lo & hi of ANNI block 0 & [MISC x3 < T4p]  (Alg. 2 lines 12-13)
-    // SPLIT path (small problems): per (tile column task, attempt of the sweep) three rows of 32 uint4, written by
-    // mask_kernel, read by sweep_warp_kernel<..., SPLIT = 2>; split_nud / split_nup = prefix lengths they hold
-    void *mask_dev;
-    uint32_t split_nud, split_nup;
     uint32_t rr;              // right reach of the variant's footprint: 2 PCPD, 3 TCPD, 4 QCPD, 1 CPD
     uint32_t pmask_code;      // paper annihilation mask: decorrelation bound b - 0: 1/4 (lo & hi), 1: 1/2 (lo), 2: 1 (all
                               // lanes), 3: 3/4 (lo | hi), lo / hi = the planes of ANNI block 0
@@ -60,29 +56,15 @@ struct JitSlot {
     int wpb;       // warps per block the kernel was compiled for (launches with another shape use the built-in kernel)
 };
 
-// SPLIT path of one handle (small problems).  The masks of a sweep depend on (seed, t, schedule, thresholds) only, not
-// on the lattice, so mask_kernel(t + 1) runs on an auxiliary stream while the update kernel of sweep t runs on the
-// handle's stream: two mask buffers (buf[t & 1]), `held[i]` = the sweep whose masks buf[i] holds (or will hold once
-// ready[i] fires), freed[i] = the update kernel that last read buf[i] has finished.
+// Small / mid-size path of one handle (column_kernel, column_device.cuh).
 struct SplitSlot {
-    void *buf[2];          // device; buf[0] == NULL: path not used
-    uint64_t launches;
-    cudaStream_t aux;
-    cudaEvent_t ready[2], freed[2];
-    int64_t held[2];       // -1: nothing
-    bool freed_valid[2];
-    int block_mode;        // 1: SPLIT = 3 instead - producer warps and the update warp in one block per tile column;
-                           // 2: column_kernel - producer warps and two half-word update warps in one block per tile column
+    uint64_t launches;     // column_kernel launches of this handle
+    int column_mode;       // 1: the handle's sweeps run column_kernel (one block per tile column)
 };
 bool column_supported(uint32_t Ts, uint32_t D);
-bool split_block_supported(uint32_t Ts, uint32_t D);
-int split_setup(SplitSlot *s);     // creates the stream and events (buffers are allocated by the API layer); 0 = ok
-void split_teardown(SplitSlot *s);
-size_t split_mask_bytes(const SweepParams &P);
-bool split_supported(uint32_t Ts, uint32_t D);
 
-// Launchers (all asynchronous on `stream`); return the number of kernels launched (launch_sweep: or -1 if a stream /
-// event operation of the two-kernel path failed; launch errors themselves surface in the caller's cudaGetLastError).
+// Launchers (all asynchronous on `stream`); return the number of kernels launched (launch errors surface in the
+// caller's cudaGetLastError).
 int launch_sweep(const SweepParams &P, int variant, bool force_block_kernel, cudaStream_t stream, JitSlot *jit,
                  SplitSlot *split);
 // warp-per-(tile, column) production kernel (sweep_warp.cu)

@@ -184,24 +184,11 @@ __device__ __forceinline__ uint32_t pmask_dec(uint32_t p0, uint32_t p1, uint32_t
     return code == 0u ? (p0 & p1) : code == 1u ? p0 : code == 2u ? ~0u : (p0 | p1);
 }
 
-// ---- TMA bulk copy + mbarrier (SPLIT consumer: the task's mask records are staged through shared memory) ----
-constexpr uint32_t MASK_REC_BYTES = 96u * 16u;  // one attempt: three rows of 32 uint4
-constexpr uint32_t MASK_MAX_CHUNKS = 256u;      // one bulk copy / mbarrier per sub-step (S <= MAX_SUBSTEPS = 256)
-
+// ---- mbarrier helpers (the producer / update-warp ring of column_kernel, column_device.cuh) ----
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
 }
 // (the suspend-time hint lets the hardware park the thread until the phase completes instead of returning at once:
 // a waiting warp then takes almost no issue slots from the warps it is waiting for)
@@ -280,69 +267,10 @@ __device__ __forceinline__ void prefix_spec(Mask2 &lt, Mask2 &und, const U4 *blk
     und = Mask2{ulo, uhi};
 }
 
-// Everything of attempt j of tile column `task` that does not depend on the lattice (the producer side of the two
-// SPLIT paths): the MISC block (fission-side mask, and the footprint position resolved to the tile-local index of
-// site x-1 with the sub-step's inner shift and seam), and the generic-threshold compare of the first P.split_nud
-// DIFF and P.split_nup ANNI blocks (the paper's gated mask when P.pmask_paper), written as three rows of 32 uint4:
-// rec[0] = {misc x0, x1, y0, x3}, rec[32] = {dlt, dund}, rec[64] = {plt, pund}  (rec already offset by the lane).
-__device__ __forceinline__ void produce_record(const SweepParams &P, uint32_t task, uint32_t j, uint32_t lane, uint32_t sigma,
-                                               uint4 *rec)
-{
-    const uint32_t ntiles = P.L / P.Ts;
-    const uint32_t tau = task % ntiles, wl = task / ntiles;
-    const uint32_t b = lane < P.n ? lane : 0u;
-    const RoundKeys &rk = P.rk;
-    const DomainPos dp = domain_pos(b, P.n, sigma, P.D, P.rr);
-    const PhiloxWarp pw = philox_warp_consts(P.t, P.word_offset + wl, rk);
-    const PhiloxSlot ps = philox_slot_consts((tau * P.n + b) * P.D + j, pw, rk);
-    Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-    U4 misc, blk[4];
-    // blocks in groups of four independent chains (the prefix lengths are run-time values here)
-    {
-        const uint32_t c3s[4] = {STREAM_MISC, STREAM_DIFF | 0u, STREAM_DIFF | 1u, STREAM_DIFF | 2u};
-        philox_blocks<4>(c3s, ps, pw, rk, blk);
-        misc = blk[0];
-#pragma unroll
-        for (uint32_t i = 0; i < 3; ++i)
-            if (i < P.split_nud)
-                cmp_block_sum(dlt, dund, blk[1 + i], P.tdm[2 * i], P.tdm[2 * i + 1], P.sd[2 * i], P.sd[2 * i + 1]);
-    }
-    for (uint32_t m = 3; m < P.split_nud; m += 4) {
-        const uint32_t c3s[4] = {STREAM_DIFF | m, STREAM_DIFF | (m + 1u), STREAM_DIFF | (m + 2u), STREAM_DIFF | (m + 3u)};
-        philox_blocks<4>(c3s, ps, pw, rk, blk);
-#pragma unroll
-        for (uint32_t i = 0; i < 4; ++i)
-            if (m + i < P.split_nud)
-                cmp_block_sum(dlt, dund, blk[i], P.tdm[2 * (m + i)], P.tdm[2 * (m + i) + 1], P.sd[2 * (m + i)],
-                              P.sd[2 * (m + i) + 1]);
-    }
-    if (!P.pmask_paper) {
-        for (uint32_t m = 0; m < P.split_nup; m += 4) {
-            const uint32_t c3s[4] = {STREAM_ANNI | m, STREAM_ANNI | (m + 1u), STREAM_ANNI | (m + 2u), STREAM_ANNI | (m + 3u)};
-            philox_blocks<4>(c3s, ps, pw, rk, blk);
-#pragma unroll
-            for (uint32_t i = 0; i < 4; ++i)
-                if (m + i < P.split_nup)
-                    cmp_block_sum(plt, pund, blk[i], P.tpm[2 * (m + i)], P.tpm[2 * (m + i) + 1], P.sp[2 * (m + i)],
-                                  P.sp[2 * (m + i) + 1]);
-        }
-    } else {
-        const U4 pb = philox_block(STREAM_ANNI, ps, pw, rk);
-        const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-        plt.lo = pmask_dec(pb.x0, pb.x2, P.pmask_code) & gate;
-        plt.hi = pmask_dec(pb.x1, pb.x3, P.pmask_code) & gate;
-    }
-    const uint32_t y0 = footprint_start(misc.x2, dp, P.Ts);
-    rec[0] = make_uint4(misc.x0, misc.x1, y0, misc.x3);
-    rec[32] = make_uint4(dlt.lo, dlt.hi, dund.lo, dund.hi);
-    rec[64] = make_uint4(plt.lo, plt.hi, pund.lo, pund.hi);
-}
-
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-constexpr uint32_t RING_PER_PRODUCER = 4u;   // SPLIT = 3: ring slots (records in flight) per producer warp
 
 }  // namespace
 
@@ -354,15 +282,8 @@ constexpr uint32_t RING_PER_PRODUCER = 4u;   // SPLIT = 3: ring slots (records i
 // SPEC = 1 (kernels compiled at run time by jit.cu): the thresholds are the template constants STD, STP
 // (low 32 bits of T_d, T_p; neither threshold is 2^32) instead of P.thd / P.thp and the host tables, and
 // the schedule constants T_s, D, A and the ring length L are the template constants CTS, CD, CA, CL.
-//
-// SPLIT = 2 (small problems, too few tile columns to fill the GPU): the state-independent part of every
-// attempt - MISC block and the compared prefix planes of DIFF and ANNI - has been computed for the whole
-// sweep by mask_kernel below, in parallel over all attempts, into P.mask_dev; this kernel then only reads
-// them (prefetched one attempt ahead), so that the sequential chain of a domain's D attempts per sweep is
-// ~150 cycles per attempt instead of ~1400.  Prefix lengths are then the run-time values P.split_nud /
-// P.split_nup (NU_D, NU_P unused).  Same results bit for bit.
 template <int VARIANT, int WPB, int NU_D, int NU_P, int PMODE, int PW, int SPEC = 0, uint32_t STD = 0u, uint32_t STP = 0u,
-          uint32_t CTS = 0u, uint32_t CD = 0u, uint32_t CA = 0u, uint32_t CL = 0u, int SPLIT = 0>
+          uint32_t CTS = 0u, uint32_t CD = 0u, uint32_t CA = 0u, uint32_t CL = 0u>
 __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(const __grid_constant__ SweepParams P)
 {
     extern __shared__ __align__(16) uint64_t smem[];  // WPB buffers of `stride` words
@@ -377,8 +298,8 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     const uint32_t ntiles = L / Ts;
-    const uint32_t task = SPLIT == 3 ? blockIdx.x : blockIdx.x * WPB + warp;
-    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel (but see SPLIT = 3)
+    const uint32_t task = blockIdx.x * WPB + warp;
+    if (task >= ntiles * P.W) return;  // warps are independent: no block-wide barrier in this kernel
 
     // C5 step 1: shifts from the SHIFT stream; lane j holds sigma_{k0+j} of the current group of 32 sub-steps.
     uint32_t sig_reg, Sigma;
@@ -394,74 +315,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     const uint32_t start = (uint32_t)(((uint64_t)Sigma + (uint64_t)tau * Ts) % L);
     uint64_t *g = P.lat + (size_t)wl * L;             // column wl, contiguous in the site index
     const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
-    uint64_t *buf = smem + (SPLIT == 3 ? (size_t)0 : (size_t)warp * stride);
+    uint64_t *buf = smem + (size_t)warp * stride;
     const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
     const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
     const uint32_t odd = vec ? (start & 1u) : 0u;
     uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
-    // SPLIT consumer (WPB = 1): the records of this task's J = S*A attempts (three rows of 32 uint4 each, contiguous
-    // in P.mask_dev) are brought into shared memory behind the tile buffer by TMA bulk copies, one per sub-step (A
-    // attempts), each completing on its own mbarrier, all issued up front by lane 0; the warp waits for a sub-step's
-    // records when it gets there, and reads each record one attempt ahead of its use.
-    const uint32_t nud = SPLIT >= 2 ? P.split_nud : (uint32_t)NU_D, nup = SPLIT >= 2 ? P.split_nup : (uint32_t)NU_P;
-    // SPLIT = 3 (ONE tile column per block of WPB warps): warps 1 .. WPB-1 are producers - they compute the records of
-    // the column's attempts (produce_record), attempt j by warp 1 + j mod (WPB-1), into a ring of RING_SLOTS records in shared
-    // memory behind the tile - and warp 0 is the update warp.  Per slot a `full` mbarrier (the producer's lane 0
-    // arrives once its warp has written the record) and an `empty` one (the update warp's lane 0 arrives once its
-    // warp has read it); no global mask buffer, no second kernel.
-    uint4 *ring = nullptr;
-    uint64_t *fullb = nullptr, *emptyb = nullptr;
-    constexpr uint32_t NPROD = WPB > 1 ? WPB - 1 : 1, RING_SLOTS = RING_PER_PRODUCER * NPROD;
-    if constexpr (SPLIT == 3) {
-        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
-        ring = reinterpret_cast<uint4 *>(mbase);
-        fullb = reinterpret_cast<uint64_t *>(mbase + (size_t)RING_SLOTS * MASK_REC_BYTES);
-        emptyb = fullb + RING_SLOTS;
-        if (threadIdx.x == 0) {
-            for (uint32_t c = 0; c < RING_SLOTS; ++c) {
-                mbar_init(fullb + c, 1u);
-                mbar_init(emptyb + c, 1u);
-            }
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncthreads();
-        if (warp != 0) {
-            const uint32_t J = S * A;
-            uint32_t sig = 0u, sig_group = ~0u;   // lane l holds sigma of sub-step 32 * sig_group + l
-            for (uint32_t j = warp - 1u; j < J; j += NPROD) {
-                const uint32_t kk = j / A;
-                if ((kk >> 5) != sig_group) {
-                    sig_group = kk >> 5;
-                    sig = __umulhi(philox4x32_10(32u * sig_group + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
-                }
-                const uint32_t sigma = __shfl_sync(0xffffffffu, sig, kk & 31u);
-                const uint32_t slot = j % RING_SLOTS, pass = j / RING_SLOTS;
-                mbar_wait(emptyb + slot, (pass & 1u) ^ 1u);   // (a fresh barrier passes a wait on parity 1)
-                produce_record(P, task, j, lane, sigma, ring + slot * 96u + lane);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(fullb + slot);
-            }
-            return;
-        }
-    }
-    const uint4 *mrec = nullptr;
-    uint64_t *bars = nullptr;
-    uint4 nx0{}, nx1{}, nx2{};
-    if constexpr (SPLIT == 2) {
-        const uint32_t J = S * A, cbytes = A * MASK_REC_BYTES;
-        uint8_t *mbase = reinterpret_cast<uint8_t *>(smem) + (((size_t)stride * 8u + 127u) & ~(size_t)127u);
-        bars = reinterpret_cast<uint64_t *>(mbase + (size_t)J * MASK_REC_BYTES);
-        if (lane == 0) {
-            for (uint32_t c = 0; c < S; ++c) mbar_init(bars + c, 1u);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            const uint8_t *src = reinterpret_cast<const uint8_t *>(P.mask_dev) + (size_t)task * J * MASK_REC_BYTES;
-            for (uint32_t c = 0; c < S; ++c) {
-                mbar_expect_tx(bars + c, cbytes);
-                bulk_g2s(mbase + (size_t)c * cbytes, src + (size_t)c * cbytes, cbytes, bars + c);
-            }
-        }
-        mrec = reinterpret_cast<const uint4 *>(mbase) + lane;   // (issued before the tile load so that the two overlap)
-    }
+    constexpr uint32_t nud = (uint32_t)NU_D, nup = (uint32_t)NU_P;
     if (vec) {
         const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
         const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
@@ -526,61 +385,21 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 
-    uint32_t rslot = 0u, rphase = 0u;   // SPLIT = 3: ring slot and mbarrier phase of the next record to take
-    if constexpr (SPLIT == 3) {
-        mbar_wait(fullb, 0u);
-        const uint4 *r = ring + lane;
-        nx0 = r[0]; nx1 = r[32]; nx2 = r[64];
-        __syncwarp();
-        if (lane == 0) mbar_arrive(emptyb);
-        rslot = 1u % RING_SLOTS;
-        if (RING_SLOTS == 1u) rphase = 1u;
-    }
 #pragma unroll 1
     for (uint32_t k = 0; k < S; ++k) {
-        DomainPos dp{};
-        if constexpr (SPLIT == 2) {  // this sub-step's records have landed? then fetch its first one
-            mbar_wait(bars + k, 0u);
-            nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64];
-        }
-        if constexpr (SPLIT < 2) {  // (SPLIT consumers: the producer has resolved the positions)
-            if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
-            const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
-            dp = domain_pos(b, n, sigma, D, Rr);
-        }
+        if (k != 0 && (k & 31u) == 0) sig_reg = __umulhi(philox4x32_10(k + lane, t, 0u, STREAM_SHIFT, rk).x0, D);
+        const uint32_t sigma = __shfl_sync(0xffffffffu, sig_reg, k & 31u);
+        const DomainPos dp = domain_pos(b, n, sigma, D, Rr);
 
 #pragma unroll 1
         for (uint32_t a = 0; a < A; ++a) {
             // The MISC block, the first NU_D DIFF blocks and the first NU_P ANNI blocks of an attempt do not
             // depend on the lattice state (only WHICH lanes matter does): independent Philox chains, issued
             // back to back so that the FMA pipe always has several wide multiplies in flight.
-            PhiloxSlot ps{};
-            if constexpr (SPLIT < 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
+            const PhiloxSlot ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
             U4 blks[1 + NU_D + NU_P];
             Mask2 dlt{0u, 0u}, dund{~0u, ~0u}, plt{0u, 0u}, pund{~0u, ~0u};
-            if constexpr (SPLIT == 3) {
-                // this attempt's record was taken out of the ring during the previous attempt; take the next one now
-                const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
-                if (k * A + a + 1u < S * A) {
-                    mbar_wait(fullb + rslot, rphase);
-                    const uint4 *r = ring + rslot * 96u + lane;
-                    nx0 = r[0]; nx1 = r[32]; nx2 = r[64];
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(emptyb + rslot);
-                    if (++rslot == RING_SLOTS) { rslot = 0u; rphase ^= 1u; }
-                }
-                blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
-                dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
-                plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
-            } else if constexpr (SPLIT == 2) {
-                // this attempt's record was fetched during the previous attempt; fetch the next one of the sub-step now
-                const uint4 r0 = nx0, r1 = nx1, r2 = nx2;
-                mrec += 96;
-                if (a + 1u < A) { nx0 = mrec[0]; nx1 = mrec[32]; nx2 = mrec[64]; }
-                blks[0] = U4{r0.x, r0.y, r0.z, r0.w};
-                dlt = Mask2{r1.x, r1.y}; dund = Mask2{r1.z, r1.w};
-                plt = Mask2{r2.x, r2.y}; pund = Mask2{r2.z, r2.w};
-            } else {
+            {
                 uint32_t c3s[1 + NU_D + NU_P];
                 c3s[0] = STREAM_MISC;
 #pragma unroll
@@ -593,7 +412,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             const U4 *dblk = blks + 1, *pblk = blks + 1 + NU_D;
 
             // C4: MISC block: Fm = ~lo (1 -> fission low, Alg. 1: r3 < 1/2), x2 -> position.
-            const uint32_t y0 = SPLIT >= 2 ? misc.x2 : footprint_start(misc.x2, dp, Ts);  // (SPLIT: resolved by the producer)
+            const uint32_t y0 = footprint_start(misc.x2, dp, Ts);
             const uint64_t Fm = ~lo64(misc);
             uint64_t *q = tile + y0;
             uint64_t sa = 0, sb = 0, sc = 0, se = 0, sf = 0, sg = 0;
@@ -607,9 +426,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             // DIFF and ANNI masks (C3): the unconditional planes are compared on all 64 lanes (no
             // dependence on the state), the lazy tails only on the lanes whose outcome can matter:
             // DIFF where x or x+1 is occupied, ANNI where a pair (triple) is present and Dm = 0.
-            if constexpr (SPLIT >= 2) {
-                // prefix compared by the producer
-            } else if constexpr (SPEC) {
+            if constexpr (SPEC) {
                 prefix_spec<STD, NU_D>(dlt, dund, dblk);
                 if constexpr (PMODE == 0) prefix_spec<STP, NU_P>(plt, pund, pblk);
             } else {
@@ -634,7 +451,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // T's bit of the last plane done (PW); SPEC: the prefix lt is exact, the tail's sum starts afresh
                 int32_t prev = (NU_D > 0 && !SPEC) ? (int32_t)((Td >> (32 - 2 * NU_D)) & 1u) : 0;
                 for (; m < nblkD && __any_sync(0xffffffffu, (dund.lo | dund.hi) != 0); ++m) {
-                    if constexpr (SPLIT >= 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);  // rare: tails only
                     const U4 blk = philox_block(STREAM_DIFF | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -663,7 +479,6 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 uint32_t m = nup;
                 int32_t prev = (NU_P > 0 && !SPEC) ? (int32_t)((Tp >> (32 - 2 * NU_P)) & 1u) : 0;
                 for (; m < nblkP && __any_sync(0xffffffffu, (pund.lo | pund.hi) != 0); ++m) {
-                    if constexpr (SPLIT >= 2) ps = philox_slot_consts(slot0 + k * A + a, pw, rk);
                     const U4 bk = philox_block(STREAM_ANNI | m, ps, pw, rk);
                     int32_t s0, s1;
                     if constexpr (PW || SPEC) {
@@ -682,11 +497,9 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
                 // an independent b-bit per lane (b = 1/4: the two planes of ANNI block 0 ANDed; pmask_dec) gated by
                 // ONE word-wide draw that is 1 w.p. p/b (x3 of the MISC block against floor((p/b) * 2^32)).
-                if constexpr (SPLIT < 2) {  // (SPLIT consumers: the producer has done this)
-                    const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-                    plt.lo = pmask_dec(pblk[0].x0, pblk[0].x2, P.pmask_code) & gate;
-                    plt.hi = pmask_dec(pblk[0].x1, pblk[0].x3, P.pmask_code) & gate;
-                }
+                const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
+                plt.lo = pmask_dec(pblk[0].x0, pblk[0].x2, P.pmask_code) & gate;
+                plt.hi = pmask_dec(pblk[0].x1, pblk[0].x3, P.pmask_code) & gate;
             }
             const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);
 
@@ -754,22 +567,5 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
         }
     }
 }
-
-// mask_kernel - producer of the two-kernel SPLIT path: one warp per (tile column task, attempt j of the sweep), lane =
-// domain; stores the records (produce_record) coalesced into P.mask_dev.  The blocks of a warp are evaluated one after
-// the other (run-time loop): the parallelism is across the (L / T_s) * W * D warps of the grid.  (Not part of the
-// run-time specialised build, which is for large problems.)
-#ifndef PCPD_JIT_BUILD
-__global__ void __launch_bounds__(128) mask_kernel(const __grid_constant__ SweepParams P)
-{
-    const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t J = P.S * P.A, ntiles = P.L / P.Ts;
-    const uint32_t gw = blockIdx.x * 4u + (threadIdx.x >> 5);
-    if (gw >= ntiles * P.W * J) return;
-    const uint32_t task = gw / J, j = gw - task * J;
-    const uint32_t sigma = __umulhi(philox4x32_10(j / P.A, P.t, 0u, STREAM_SHIFT, P.rk).x0, P.D);  // C5 step 1
-    produce_record(P, task, j, lane, sigma, reinterpret_cast<uint4 *>(P.mask_dev) + (size_t)gw * 96u + lane);
-}
-#endif
 
 }  // namespace pcpd

@@ -86,9 +86,8 @@ def gpu_check(pk, kw, sch, init, times, words=None, words_in=None, expect_jit=Fa
             pytest.skip("libnvrtc is not installed on this box: the built-in kernel ran (and passed the checks above)")
         assert g.jit_state() == 1, pk.jit_message()
     if expect_split is not None:  # which small-problem path ran: launches per handle on the SPLIT paths
-        # "force": two-kernel path (one update kernel per sweep + one mask_kernel per sweep, the next sweep's being
-        # launched one sweep ahead); "column" / "block": one kernel per sweep; False: the fused kernel
-        want = 0 if not expect_split else times[-1] if expect_split in ("block", "column") else 2 * times[-1] + 1
+        # "column": one column_kernel per sweep; False: the fused kernel
+        want = times[-1] if expect_split else 0
         assert g.split_launch_count() == want
     g.close()
 
@@ -141,13 +140,12 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("split", ["auto", "0", "force", "block"])
+@pytest.mark.parametrize("split", ["auto", "0"])
 @pytest.mark.parametrize("case", SMALL, ids=[f"case{i}" for i in range(len(SMALL))])
 def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
     """Every word and count after every sweep.  split = auto: these sizes run column_kernel (producer warps + two
     half-word update warps in one block per tile column) wherever the warp kernel applies (at most 32 domains per tile);
-    split = 0: the fused warp kernel (or the generic block kernel for more than 32 domains per tile); force / block: the
-    two earlier small-problem forms (mask_kernel + update kernel; four-warp producer / consumer block)."""
+    split = 0: the fused warp kernel (or the generic block kernel for more than 32 domains per tile)."""
     variant, L, R, d, p, Ts, D, A, init = case
     if split != "auto":
         monkeypatch.setenv("PCPD_SPLIT", split)
@@ -251,25 +249,23 @@ def test_mid_size_handle_runs_the_column_kernel(pk):
     gpu_check(pk, kw, {}, 1, [1, 2], words=[31], expect_split=False)
 
 
-def test_two_kernel_path_mask_prefetch_bookkeeping(pk, monkeypatch):
-    """The two-kernel small-problem path (PCPD_SPLIT=force) produces the masks of sweep t+1 one sweep ahead on an auxiliary stream
-    (double-buffered).  Re-initialising, and setting the sweep counter backwards, forwards or to the value already
-    prefetched, must give what the fused kernel gives for the same sequence of calls."""
+def test_counter_jumps_and_reinit_on_the_column_kernel(pk, monkeypatch):
+    """Re-initialising and setting the sweep counter backwards, forwards and to the last legal sweep must give what the
+    fused kernel gives for the same sequence of calls (lattice + counter is the whole state, C7)."""
     def sequence(g):
         out = []
         g.init(1); g.run(3); out.append(g.get_lattice())
-        g.init(1); g.run(2); out.append(g.get_lattice())      # counter back to 0 with stale prefetched masks
+        g.init(1); g.run(2); out.append(g.get_lattice())
         g.sweep = 9; g.run(1); g.run(2); out.append(g.get_lattice())
-        g.sweep = 12; g.run(1); out.append(g.get_lattice())   # counter set to the sweep whose masks are already there
         g.sweep = 4; g.run(3); out.append(g.get_lattice())
-        g.sweep = 2 ** 32 - 2; g.run(1); out.append(g.get_lattice())   # last legal sweep: nothing to prefetch
+        g.sweep = 2 ** 32 - 2; g.run(1); out.append(g.get_lattice())   # last legal sweep
         return out
     res = []
-    for mode in ("force", "0"):
+    for mode in ("1", "0"):
         monkeypatch.setenv("PCPD_SPLIT", mode)
         g = pk.Pcpd(4096, 192, 0.3, 0.12, 11, 0)
         res.append(sequence(g))
-        assert (g.split_launch_count() > 0) == (mode == "force")
+        assert (g.split_launch_count() > 0) == (mode == "1")
         g.close()
     for x, y in zip(*res):
         assert np.array_equal(x, y)
