@@ -38,7 +38,7 @@ EXPORTS = (
     "pcpd_thresholds", "pcpd_sweep", "pcpd_set_sweep", "pcpd_synchronize", "pcpd_destroy", "pcpd_last_error",
     "pcpd_launch_count", "pcpd_microbench", "pcpd_jit_state", "pcpd_jit_message", "pcpd_jit_launch_count",
     "pcpd_jit_selftest", "pcpd_split_launch_count", "pcpd_step_from_host", "pcpd_run_series", "pcpd_delta_eff",
-    "pcpd_run_series_static",
+    "pcpd_run_series_static", "pcpd_step_from_host_columns",
 )
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -126,6 +126,8 @@ def load_library() -> C.CDLL:
     L.pcpd_run_series.restype = C.c_int
     L.pcpd_step_from_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     L.pcpd_step_from_host.restype = C.c_int
+    L.pcpd_step_from_host_columns.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+    L.pcpd_step_from_host_columns.restype = C.c_int
     L.pcpd_split_launch_count.argtypes = [C.c_void_p]
     L.pcpd_split_launch_count.restype = C.c_uint64
     L.pcpd_run_series_static.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
@@ -313,6 +315,10 @@ class Pcpd:
     def step_from_host_ptr(self, host_lattice_ptr: int, n_sweeps: int, host_counts_ptr: int = 0):
         """set_lattice + run(n_sweeps) + density with the upload pipelined against the sweeps (pcpd_step_from_host)."""
         _check(self._lib, self._lib.pcpd_step_from_host(self._h, host_lattice_ptr, int(n_sweeps), host_counts_ptr or None))
+
+    def step_from_host_columns_ptr(self, host_columns_ptr: int, n_sweeps: int, host_counts_ptr: int = 0):
+        """pcpd_step_from_host_columns: the same step from a column-major host lattice [w][i] (contiguous chunk copies)."""
+        _check(self._lib, self._lib.pcpd_step_from_host_columns(self._h, host_columns_ptr, int(n_sweeps), host_counts_ptr or None))
 
     def density_ptr(self, host_ptr: int):
         _check(self._lib, self._lib.pcpd_density(self._h, host_ptr))

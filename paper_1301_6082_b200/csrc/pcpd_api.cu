@@ -651,21 +651,9 @@ static uint32_t step_chunk_columns(const pcpd_t *h)
     return 8u;
 }
 
-int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, uint32_t *out_counts)
+// copy stream and per-chunk events of the pipelined steps: created on first use, kept for the life of the handle
+static int ensure_copy_resources(pcpd_t *h, uint32_t nchunks)
 {
-    if (!h || !in_words) return fail(PCPD_ERR_ARG, "null argument");
-    if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
-    const uint32_t cw = step_chunk_columns(h);
-    const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
-    if (cw >= W || h->thr || h->force_block) {   // no pipelining: the plain sequence
-        int rc = pcpd_set_lattice(h, in_words);
-        if (rc == PCPD_OK) rc = pcpd_run(h, n_sweeps);
-        if (rc == PCPD_OK && out_counts) rc = pcpd_density(h, out_counts);
-        return rc;
-    }
-    const size_t bytes = 8 * h->L * h->W;
-    const uint32_t nchunks = (W + cw - 1) / cw;
-    // copy stream and events: created on first use, kept for the life of the handle
     cudaError_t e = cudaSuccess;
     if (!h->copy_stream) e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess && !h->copy_start) e = cudaEventCreateWithFlags(&h->copy_start, cudaEventDisableTiming);
@@ -680,6 +668,87 @@ int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, 
         if (e != cudaSuccess) --h->n_chunk_ev;   // (the slot of the failed creation holds nothing)
     }
     if (e != cudaSuccess) return cuda_fail(e, "step_from_host: copy stream / events");
+    return PCPD_OK;
+}
+
+// Column-major host buffer (the device's own layout): chunks of columns are contiguous, so every chunk is ONE plain copy
+// straight into the lattice - no staging buffer, no transpose - at the full host-to-device rate.
+int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t n_sweeps, uint32_t *out_counts)
+{
+    if (!h || !in_columns) return fail(PCPD_ERR_ARG, "null argument");
+    if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
+    // chunk: as few columns as still fill the GPU with one launch (2 blocks of 7 warps per SM, twice over), so that the
+    // first, exposed copy is short; handles that cannot be chunked that way copy the whole lattice first
+    uint32_t cw = W;
+    if (const char *e = getenv("PCPD_STEP_CHUNK")) {   // tuning hook: columns per chunk (0 = no pipelining)
+        const long v = atol(e);
+        cw = v <= 0 || (uint64_t)v >= h->W ? W : (uint32_t)v;
+    } else if (!h->thr && !h->force_block) {
+        const uint64_t per_col = h->L / h->Ts;
+        if (per_col > 0) {
+            const uint64_t want = (4ull * 148 * 14 + per_col - 1) / per_col;
+            if (want * 2 <= W) cw = (uint32_t)want;
+        }
+    }
+    if (h->thr || h->force_block) cw = W;
+    const uint32_t nchunks = (W + cw - 1) / cw;
+    int rc = ensure_copy_resources(h, nchunks);
+    if (rc != PCPD_OK) return rc;
+    cudaStream_t copy = h->copy_stream;
+    cudaEvent_t *ev = h->chunk_ev;
+    h->invalid = true;   // the lattice is overwritten chunk by chunk (see pcpd_step_from_host)
+    cudaError_t e = cudaEventRecord(h->copy_start, h->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, h->copy_start, 0);
+    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
+        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        e = cudaMemcpyAsync(h->lat + (size_t)w0 * L, in_columns + (size_t)w0 * L, (size_t)nw * L * 8, cudaMemcpyHostToDevice, copy);
+        if (e == cudaSuccess) e = cudaEventRecord(ev[c], copy);
+    }
+    for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
+        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        e = cudaStreamWaitEvent(h->stream, ev[c], 0);
+        if (e != cudaSuccess) break;
+        SweepParams Pc = h->P;   // the chunk as a lattice of its own: columns w0 .. w0+nw-1 (columns never interact)
+        Pc.lat = h->lat + (size_t)w0 * L;
+        Pc.W = nw;
+        Pc.word_offset = h->P.word_offset + w0;
+        if (h->thr) Pc.thr_dev = h->thr + 4 * (size_t)w0;
+        for (uint64_t it = 0; it < n_sweeps; ++it) {
+            Pc.t = (uint32_t)(h->sweep + it);
+            g_launches += launch_sweep(Pc, h->variant, h->force_block, h->stream, &h->jit, nchunks == 1 ? &h->split : nullptr);
+        }
+    }
+    if (e == cudaSuccess) rc = check_launch("pipelined step");
+    if (e == cudaSuccess && rc == PCPD_OK) {
+        h->sweep += n_sweeps;
+        h->invalid = false;
+        if (out_counts) rc = pcpd_density(h, out_counts);
+        else e = cudaStreamSynchronize(h->stream);
+    }
+    cudaStreamSynchronize(copy);
+    cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "step_from_host_columns");
+    return rc;
+}
+
+int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n_sweeps, uint32_t *out_counts)
+{
+    if (!h || !in_words) return fail(PCPD_ERR_ARG, "null argument");
+    if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
+    const uint32_t cw = step_chunk_columns(h);
+    const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
+    if (cw >= W || h->thr || h->force_block) {   // no pipelining: the plain sequence
+        int rc = pcpd_set_lattice(h, in_words);
+        if (rc == PCPD_OK) rc = pcpd_run(h, n_sweeps);
+        if (rc == PCPD_OK && out_counts) rc = pcpd_density(h, out_counts);
+        return rc;
+    }
+    const size_t bytes = 8 * h->L * h->W;
+    const uint32_t nchunks = (W + cw - 1) / cw;
+    int rc0 = ensure_copy_resources(h, nchunks);
+    if (rc0 != PCPD_OK) return rc0;
+    cudaError_t e = cudaSuccess;
     uint64_t *stage = (uint64_t *)dev_alloc(h->mem, bytes, h->stream);
     if (!stage) return fail(PCPD_ERR_ALLOC, "staging allocation failed");
     cudaStream_t copy = h->copy_stream;

@@ -289,8 +289,21 @@ def test_pipelined_step_from_host_equals_the_plain_sequence(pk, monkeypatch):
     o = oracle.Oracle(L, R, 0.3, 0.12, 21, 0)
     o.set_words(w0); o.sweep = 5; o.run(3)
     assert np.array_equal(b.get_lattice(), o.get_words()) and np.array_equal(cnt, o.counts())
-    a.close(); b.close()
+    # the column-major variant (contiguous chunk copies straight into the lattice), same forced ragged chunks
+    c2 = pk.Pcpd(L, R, 0.3, 0.12, 21, 0)
+    c2.sweep = 5
+    cols = np.ascontiguousarray(w0.T)
+    cnt2 = np.empty(R, dtype=np.uint32)
+    c2.step_from_host_columns_ptr(cols.ctypes.data, 3, cnt2.ctypes.data)
+    assert c2.sweep == 8 and np.array_equal(c2.get_lattice(), o.get_words()) and np.array_equal(cnt2, o.counts())
+    a.close(); b.close(); c2.close()
     monkeypatch.delenv("PCPD_STEP_CHUNK")
+    # unchunked (small handle: the column kernel runs), per-word thresholds
+    s1 = pk.Pcpd(L, R, 0.3, 0.12, 21, 0)
+    s1.sweep = 5
+    s1.step_from_host_columns_ptr(cols.ctypes.data, 3, cnt2.ctypes.data)
+    assert np.array_equal(s1.get_lattice(), o.get_words()) and np.array_equal(cnt2, o.counts()) and s1.split_launch_count() == 3
+    s1.close()
     c = wl.BY_NAME["cfg5"]
     import torch
     host = torch.empty((c.L, c.W), dtype=torch.int64).pin_memory()
@@ -302,7 +315,13 @@ def test_pipelined_step_from_host_equals_the_plain_sequence(pk, monkeypatch):
     cnt = np.empty(c.n_replicas, dtype=np.uint32)
     b.step_from_host_ptr(host.data_ptr(), 2, cnt.ctypes.data)
     assert np.array_equal(a.get_lattice(), b.get_lattice()) and np.array_equal(a.density(), cnt)
-    a.close(); b.close()
+    hostc = torch.empty((c.W, c.L), dtype=torch.int64).pin_memory()
+    hostc.numpy().view(np.uint64)[:] = hn.T
+    d = pk.Pcpd(c.L, c.n_replicas, c.d, c.p, c.seed, c.variant)
+    cnt3 = np.empty(c.n_replicas, dtype=np.uint32)
+    d.step_from_host_columns_ptr(hostc.data_ptr(), 2, cnt3.ctypes.data)     # default chunking: 3 columns of 512 tiles each
+    assert np.array_equal(a.get_lattice(), d.get_lattice()) and np.array_equal(cnt, cnt3)
+    a.close(); b.close(); d.close()
 
 
 def test_run_series_equals_run_and_density_in_a_loop(pk):
