@@ -678,8 +678,8 @@ int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t 
     if (!h || !in_columns) return fail(PCPD_ERR_ARG, "null argument");
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
-    // chunk: as few columns as still fill the GPU with one launch (2 blocks of 7 warps per SM, twice over), so that the
-    // first, exposed copy is short; handles that cannot be chunked that way copy the whole lattice first
+    // chunk: as few columns as still give a launch two full waves of warps (2 x 148 SMs x 14 warps), so that the first,
+    // exposed copy is short; handles too small for two such chunks copy the whole lattice first
     uint32_t cw = W;
     if (const char *e = getenv("PCPD_STEP_CHUNK")) {   // tuning hook: columns per chunk (0 = no pipelining)
         const long v = atol(e);
@@ -687,8 +687,8 @@ int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t 
     } else if (!h->thr && !h->force_block) {
         const uint64_t per_col = h->L / h->Ts;
         if (per_col > 0) {
-            const uint64_t want = (4ull * 148 * 14 + per_col - 1) / per_col;
-            if (want * 2 <= W) cw = (uint32_t)want;
+            const uint64_t want = (2ull * 148 * 14 + per_col - 1) / per_col;
+            if (want < W) cw = (uint32_t)want;
         }
     }
     if (h->thr || h->force_block) cw = W;

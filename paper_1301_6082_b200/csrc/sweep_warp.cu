@@ -167,7 +167,7 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
             // prefix lengths of the specialised kernel: all of a short threshold's blocks, else 6 DIFF / 4 ANNI (5 for
             // TCPD and QCPD) (tuned on B200 at cfg3-5: its prefix compare is cheaper than the built-in kernel's)
             JitSpec js;
-            js.variant = variant; js.wpb = wpb; js.pmode = P.pmask_paper ? 1 : 0;
+            js.variant = variant; js.wpb = wpb; js.pmode = P.pmask_paper ? 2 + (int)P.pmask_code : 0;   // (bound code baked in)
             js.nud = (int)min((P.thd.nplanes + 1) >> 1, 6u);
             js.nup = P.pmask_paper ? 1 : (int)min((P.thp.nplanes + 1) >> 1, variant == 1 || variant == 2 ? 5u : 4u);
             if (const char *e = getenv("PCPD_JIT_NUD")) js.nud = atoi(e);   // tuning hooks

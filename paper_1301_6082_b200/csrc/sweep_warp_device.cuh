@@ -497,9 +497,12 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 // The paper's own annihilation mask (Alg. 2 lines 12-13):
                 // an independent b-bit per lane (b = 1/4: the two planes of ANNI block 0 ANDed; pmask_dec) gated by
                 // ONE word-wide draw that is 1 w.p. p/b (x3 of the MISC block against floor((p/b) * 2^32)).
+                // (PMODE = 1: bound code from P.pmask_code; PMODE = 2 .. 5, the run-time specialised kernels: code PMODE - 2
+                // as a compile-time constant, so that the select folds away)
+                const uint32_t code = PMODE >= 2 ? (uint32_t)(PMODE - 2) : P.pmask_code;
                 const uint32_t gate = misc.x3 < P.T4p ? ~0u : 0u;
-                plt.lo = pmask_dec(pblk[0].x0, pblk[0].x2, P.pmask_code) & gate;
-                plt.hi = pmask_dec(pblk[0].x1, pblk[0].x3, P.pmask_code) & gate;
+                plt.lo = pmask_dec(pblk[0].x0, pblk[0].x2, code) & gate;
+                plt.hi = pmask_dec(pblk[0].x1, pblk[0].x3, code) & gate;
             }
             const uint64_t Pm = (PMODE == 0 && allP) ? ~0ull : m64(plt);
 
