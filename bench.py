@@ -303,8 +303,8 @@ def measure_resident(pk, torch, cfg: wl.Config, rank: int, steps: int, warmup: i
 
 
 def jit_expected(cfg: wl.Config) -> bool:
-    """Handles with at least 148 x 14 tile columns run the run-time specialised kernel."""
-    return (cfg.L // min(cfg.L, 2048)) * cfg.W >= 148 * 14 and os.environ.get("PCPD_JIT", "1") != "0"
+    """Handles with more than 768 tile columns run the run-time specialised kernel."""
+    return (cfg.L // min(cfg.L, 2048)) * cfg.W > 768 and os.environ.get("PCPD_JIT", "1") != "0"
 
 
 def ours_arm(args, cfg: wl.Config) -> None:

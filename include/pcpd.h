@@ -234,8 +234,8 @@ PCPD_API const char *pcpd_last_error(void);              /* thread-local, librar
 
 /* ---- run-time specialisation of the sweep kernel -------
  * d and p are constants for the life of a handle, and the kernel's compare of the random planes with
- * the bits of T_d, T_p (C3) is cheaper when those bits are compile-time constants.  For large problems
- * (at least 148 x 14 tile columns) the first pcpd_run of a handle therefore compiles the SAME device
+ * the bits of T_d, T_p (C3) is cheaper when those bits are compile-time constants.  For handles with more
+ * tile columns than that limit (smaller ones run column_kernel) the first pcpd_run of a handle therefore compiles the SAME device
  * source with T_d, T_p - and the schedule constants T_s, D, A and L - as template constants (NVRTC,
  * sm_100a; about a second, once per process, device and parameter set) and runs that kernel from then on.  Results are identical bit for bit.  If
  * libnvrtc cannot be loaded or the compilation fails, the handle keeps the built-in generic-threshold
@@ -257,8 +257,8 @@ PCPD_API int pcpd_jit_selftest(int variant, uint32_t T_d, uint32_t T_p, uint64_t
 
 /* ---- small and mid-size problems: one block per tile column -----------
  * With fewer tile columns ((L / T_s) * W) than the GPU has warp slots to fill, one warp per tile column leaves the
- * machine idle and each sweep is the latency of one warp's chain of D attempts.  Handles with at most 512 tile columns
- * therefore run column_kernel: one block per tile column in which producer warps compute the state-independent part
+ * machine idle and each sweep is the latency of one warp's chain of D attempts.  Handles with at most 768 tile columns
+ * (384 or 296 when the thresholds need few random planes) therefore run column_kernel: one block per tile column in which producer warps compute the state-independent part
  * of every attempt (MISC block, footprint position, the complete masks Dm and Pm) into a shared-memory ring and two
  * update warps - one per 32-bit half of the 64 replica lanes, which never interact - apply the attempts in order.
  * Same results bit for bit.  Environment, read by pcpd_create*: PCPD_SPLIT=0 never (the fused kernel at every size);

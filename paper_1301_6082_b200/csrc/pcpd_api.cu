@@ -310,12 +310,14 @@ pcpd_t *pcpd_create_ex(uint64_t L, uint64_t n_replicas, double d, double p, uint
         // (column_device.cuh): one block per tile column, producer warps computing the state-independent part of every
         // attempt, two update warps (one per 32-bit half of the replica lanes) applying them in order.  Measured on B200
         // at L = 65536, generic thresholds, per sweep (fused warp kernel -> column kernel): 128 columns 75 -> 18.6 us,
-        // 256: 76 -> 31 us, 512: 76 -> 57 us, 1024: 101 -> 96 us; from there on the fused kernel is as fast or faster.
-        // PCPD_SPLIT: unset / "1" auto (up to 512 tile columns); "0" never; "column" at every size (test hook).
+        // 256: 76 -> 31 us, 512: 76 -> 57 us, 768: 91 -> 82 us; the limit (column_task_limit, sweep_warp.cu) is lower for
+        // thresholds that need few Philox blocks.
+        // PCPD_SPLIT: unset / "1" auto; "0" never; "column" at every size (test hook).
         const char *sm = getenv("PCPD_SPLIT");
         const int mode = !sm ? 1 : !strcmp(sm, "0") ? 0 : !strcmp(sm, "column") ? 2 : 1;
         const uint64_t ntasks = (L / Ts) * W;
-        if ((mode == 2 || (mode == 1 && ntasks <= 512)) && column_supported(Ts, D) && !h->force_block) h->split.column_mode = 1;
+        if ((mode == 2 || (mode == 1 && ntasks <= column_task_limit(P))) && column_supported(Ts, D) && !h->force_block)
+            h->split.column_mode = 1;
     }
     g_err[0] = 0;
     return h;
@@ -504,7 +506,7 @@ static bool next_sweep_would_compile(const pcpd_s *h)
     if (!sweep_warp_supported(h->Ts, h->D)) return false;
     if (h->jit.mode != 2 && h->split.column_mode) return false;
     if (h->P.thd.all || h->P.thp.all) return false;
-    return h->jit.mode == 2 || sweep_warp_wpb(h->Ts, (h->L / h->Ts) * h->W) == 7;
+    return h->jit.mode == 2 || (h->L / h->Ts) * h->W > column_task_limit(h->P);
 }
 
 int pcpd_run_series_static(pcpd_t *h, const uint64_t *times, uint64_t n_times, uint32_t *out_counts, uint32_t *out_pairs)

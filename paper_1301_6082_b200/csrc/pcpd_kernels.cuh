@@ -62,6 +62,7 @@ struct SplitSlot {
     int column_mode;       // 1: the handle's sweeps run column_kernel (one block per tile column)
 };
 bool column_supported(uint32_t Ts, uint32_t D);
+uint64_t column_task_limit(const SweepParams &P);   // up to this many tile columns column_kernel is the default
 
 // Launchers (all asynchronous on `stream`); return the number of kernels launched (launch errors surface in the
 // caller's cudaGetLastError).

@@ -87,6 +87,18 @@ static size_t column_smem_bytes(uint32_t Ts, uint32_t nprod)
 
 bool column_supported(uint32_t Ts, uint32_t D) { return Ts / D <= 32 && column_smem_bytes(Ts, 2) <= 226 * 1024; }
 
+// Up to how many tile columns column_kernel beats the fused warp kernel (run-time specialised) - measured on B200 at
+// L = 65536: its time grows with the blocks per SM, the fused kernel's only with the waves of 592
+// warps, and the fewer Philox blocks the thresholds need, the earlier the fused kernel wins: both thresholds long
+// (generic d and p) 768 columns (82 vs 91 us); one long (d = 1/2, generic p; also TCPD) 384 (35 vs 37 us; 512: 42 vs 37);
+// none (dyadic d with the paper's annihilation mask) 296 = two blocks per SM (16 vs 21 us; 384: 31 vs 21).
+uint64_t column_task_limit(const SweepParams &P)
+{
+    const bool long_d = ((P.thd.nplanes + 1u) >> 1) >= (uint32_t)5;
+    const bool long_p = !P.pmask_paper && ((P.thp.nplanes + 1u) >> 1) >= (uint32_t)5;
+    return long_d && long_p ? 768u : (long_d || long_p) ? 384u : 296u;
+}
+
 // producer warps per block (measured on B200 at L = 65536, generic thresholds): 14 (a 16-warp
 // block) while every tile column has an SM of its own - cfg2: 18.6 us per sweep with 14, 20.5 with 8, 26.6 with 4 -
 // and 8 (a 10-warp block, six of which share an SM) beyond: 256 columns 30.8 us (4: 33.2, 14: 34.9), 512 columns
@@ -159,10 +171,13 @@ int launch_sweep_warp(const SweepParams &P, int variant, int wpb, cudaStream_t s
     if (split && split->column_mode && !(jit && jit->mode == 2)) return launch_sweep_column(P, variant, stream, split);
     const int nup = P.pmask_paper ? -1 : nu_p_of((P.thp.nplanes + 1) >> 1);
     const int nud = nu_d_of((P.thd.nplanes + 1) >> 1);
-    // Threshold-specialised kernel (jit.cu): large problems (wpb == 7), or every size with PCPD_JIT=force.  Not
+    // Threshold-specialised kernel (jit.cu): every handle the fused kernel serves by default (more tile columns than
+    // column_task_limit; measured 9-10 % faster than the built-in kernel at 1024 and 2048 columns too), or every size with
+    // PCPD_JIT=force.  Not
     // for T = 2^32 (d = 1 or p = 1; the template constants hold 32 bits).  If it cannot be had, the built-in
     // kernel below computes the same thing.
-    if (jit && jit->mode && jit->state >= 0 && (jit->mode == 2 || wpb == 7) && !P.thd.all && !P.thp.all) {
+    const uint64_t ntasks_all = (uint64_t)(P.L / P.Ts) * P.W;
+    if (jit && jit->mode && jit->state >= 0 && (jit->mode == 2 || ntasks_all > column_task_limit(P)) && !P.thd.all && !P.thp.all) {
         if (jit->state == 0) {
             // prefix lengths of the specialised kernel: all of a short threshold's blocks, else 6 DIFF / 4 ANNI (5 for
             // TCPD and QCPD) (tuned on B200 at cfg3-5: its prefix compare is cheaper than the built-in kernel's)

@@ -240,13 +240,18 @@ def test_invariants_on_gpu(pk):
 
 
 def test_mid_size_handle_runs_the_column_kernel(pk):
-    """Up to 512 tile columns the default is column_kernel, with 8 producer warps per block from 149 columns on (several
-    blocks share an SM): sampled columns against the oracle at 256 and 512 tile columns; 1024 run the fused kernel."""
-    for W, words in ((8, [0, 5, 7]), (16, [3, 15])):   # 32 tiles x W columns
+    """Up to 768 tile columns (generic thresholds; 384 with one short threshold) the default is column_kernel, with 8
+    producer warps per block from 149 columns on (several blocks share an SM): sampled columns against the oracle at 256
+    and 768 tile columns; above the limit the handle runs the fused kernel, run-time specialised."""
+    for W, words in ((8, [0, 5, 7]), (24, [3, 23])):   # 32 tiles x W columns
         kw = dict(L=65536, n_replicas=64 * W, d=0.1, p=0.09, seed=2, variant=0)
         gpu_check(pk, kw, {}, 1, [1, 2, 3], words=words, expect_split="column")
-    kw = dict(L=65536, n_replicas=64 * 32, d=0.1, p=0.09, seed=2, variant=0)
-    gpu_check(pk, kw, {}, 1, [1, 2], words=[31], expect_split=False)
+    kw = dict(L=65536, n_replicas=64 * 32, d=0.1, p=0.09, seed=2, variant=0)       # 1024 columns
+    gpu_check(pk, kw, {}, 1, [1, 2], words=[31], expect_split=False, expect_jit=True)
+    kw = dict(L=65536, n_replicas=64 * 16, d=0.5, p=0.152, seed=3, variant=0)      # 512 columns, d = 1/2: above its limit of 384
+    gpu_check(pk, kw, {}, 0, [1, 2], words=[0, 15], expect_split=False, expect_jit=True)
+    kw = dict(L=65536, n_replicas=64 * 12, d=0.5, p=0.152, seed=3, variant=0)      # 384 columns, d = 1/2: column kernel
+    gpu_check(pk, kw, {}, 0, [1, 2], words=[11], expect_split="column")
 
 
 def test_counter_jumps_and_reinit_on_the_column_kernel(pk, monkeypatch):
