@@ -26,6 +26,12 @@
 #pragma once
 #include "pcpd_kernels.cuh"
 
+// 1: the tile column of sweep_warp_kernel moves between HBM and shared memory by TMA bulk copies (cp.async.bulk);
+// 0: by a coalesced 128-bit load / store loop of the warp (the round-1 form; -DPCPD_TMA_TILE=0 to compare)
+#ifndef PCPD_TMA_TILE
+#define PCPD_TMA_TILE 1
+#endif
+
 namespace pcpd {
 
 namespace {
@@ -190,6 +196,23 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
+// TMA bulk copies (1-D, cp.async.bulk) of a tile column between global and shared memory: addresses and sizes are
+// multiples of 16 bytes; the load completes on an mbarrier (complete_tx), the store is tracked as a bulk group.
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+
 // (the suspend-time hint lets the hardware park the thread until the phase completes instead of returning at once:
 // a waiting warp then takes almost no issue slots from the warps it is waiting for)
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
@@ -323,6 +346,21 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     constexpr uint32_t nud = (uint32_t)NU_D, nup = (uint32_t)NU_P;
     if (vec) {
         const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
+#if PCPD_TMA_TILE
+        // the warp's tile column (16-byte aligned: s0, L even) by TMA bulk copy - two pieces where it passes the ring
+        // wrap - completing on the warp's own mbarrier: the copy engine moves the 16 KB, the warp issues 2 instructions
+        __shared__ __align__(8) uint64_t tile_bar[WPB];
+        if (lane == 0) {
+            mbar_init(&tile_bar[warp], 1u);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            const uint32_t nwords = 2u * npairs, first = min(nwords, L - s0);
+            mbar_expect_tx(&tile_bar[warp], nwords * 8u);
+            bulk_g2s(buf, g + s0, first * 8u, &tile_bar[warp]);
+            if (first < nwords) bulk_g2s(buf + first, g, (nwords - first) * 8u, &tile_bar[warp]);
+        }
+        __syncwarp();
+        mbar_wait(&tile_bar[warp], 0u);
+#else
         const ulonglong2 *g2 = reinterpret_cast<const ulonglong2 *>(g);
         ulonglong2 *b2 = reinterpret_cast<ulonglong2 *>(buf);
 #pragma unroll 8
@@ -331,6 +369,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
             if (i >= L) i -= L;
             b2[pi] = g2[i >> 1];
         }
+#endif
         if (conn && s0 + 2 * npairs > L) {
             // connected lattice: rotate the words past the ring wrap in place (L and s0 are even, so
             // both words of a pair lie on the same side of the wrap)
@@ -548,6 +587,29 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     }
     if (vec) {
         const uint32_t s0 = start - odd, npairs = Ts / 2 + odd;
+#if PCPD_TMA_TILE
+        // TMA bulk store of the 16-byte-aligned part of the buffer; an odd-aligned tile holds one foreign word at either
+        // end of its buffer: those two edge pairs are left out of the bulk copy and their own words stored by hand
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every lane: its generic-proxy writes -> async proxy
+        __syncwarp();                                                   // ... all of them before lane 0 issues the copy
+        if (lane == 0) {
+            const uint32_t w0 = 2u * odd, w1 = 2u * npairs - 2u * odd;   // buffer words [w0, w1) go by bulk copy
+            uint32_t i0 = s0 + w0;
+            if (i0 >= L) i0 -= L;
+            const uint32_t first = min(w1 - w0, L - i0);
+            bulk_s2g(g + i0, buf + w0, first * 8u);
+            if (first < w1 - w0) bulk_s2g(g, buf + w0 + first, (w1 - w0 - first) * 8u);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            if (odd) {
+                uint32_t ia = s0 + 1u, ib = s0 + 2u * npairs - 2u;
+                if (ia >= L) ia -= L;
+                if (ib >= L) ib -= L;
+                g[ia] = buf[1];
+                g[ib] = buf[2u * npairs - 2u];
+            }
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is read before the warp exits
+        }
+#else
         ulonglong2 *g2 = reinterpret_cast<ulonglong2 *>(g);
         const ulonglong2 *b2 = reinterpret_cast<const ulonglong2 *>(buf);
 #pragma unroll 8
@@ -562,6 +624,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
                 g2[i >> 1] = b2[pi];
             }
         }
+#endif
     } else {
         for (uint32_t y = lane; y < Ts; y += 32) {
             uint32_t i = start + y;
