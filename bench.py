@@ -35,7 +35,7 @@ import workloads as wl
 SWEEPS_PER_STEP = 10
 # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, a CONSTANT copied from the committed
 # `ncu --set full` capture named beside it (not measured by this run; re-captured when the kernel changes)
-NCU_TRAFFIC_BYTES = {"cfg4": (2.090e9, "profiles/r2_sweep_kernel_full.md: 1.074 GB read + 1.016 GB written per launch")}
+NCU_TRAFFIC_BYTES = {"cfg4": (2.088e9, "profiles/r2_sweep_kernel_full.md: 1.074 GB read + 1.014 GB written per launch")}
 METRIC = "replica_site_updates_per_sec"
 UNIT = "replica-site updates/s"
 
