@@ -137,6 +137,8 @@ SMALL = [
     (0x500, 4096, 256, 0.75, 0.4, 2048, 64, 4, 0),   # the paper's mask family: bound b = 1/2 (one raw word), p < 1/2
     (0x900, 2048, 192, 0.3, 0.6, 512, 64, 8, 1),     # b = 1: no decorrelation bits, fully correlated lanes
     (0xD01, 4096, 128, 0.5, 0.7, 2048, 64, 4, 0),    # b = 3/4 (two raw words ORed, gate 4p/3) on TCPD
+    (0, 4096, 128, 0.5, 0.15, 2048, 256, 8, 0),      # SD2(2048, 256, 8): the schedule without measurable bias; 8 domains per tile
+    (0, 8192, 64, 0.8, 0.12, 2048, 128, 4, 1),       # SD2(2048, 128, 4): 16 domains per tile, S = 32 sub-steps
 ]
 
 
@@ -156,7 +158,7 @@ def test_small_cases_bit_exact_every_sweep(pk, case, split, monkeypatch):
 
 
 # cases of SMALL the warp kernel runs (at most 32 domains per tile) with neither threshold equal to 2^32
-JIT_CASES = [0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12, 14, 16, 17, 18, 19, 20, 22, 23, 25, 26, 27, 29, 31, 32, 33]
+JIT_CASES = [0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12, 14, 16, 17, 18, 19, 20, 22, 23, 25, 26, 27, 29, 31, 32, 33, 34, 35]
 
 
 @pytest.mark.parametrize("idx", JIT_CASES, ids=[f"case{i}" for i in JIT_CASES])
