@@ -3,8 +3,9 @@
 // Mapping: ONE WARP owns one (tile, word column) for a whole sweep; LANE b owns
 // domain b of that tile (n = T_s / D <= 32 domains).  The column's T_s words
 // live in shared memory from load to store, so the lattice crosses HBM exactly
-// once in each direction per sweep (0.25 B per replica-site update), with
-// coalesced 128-bit global accesses.  Because all domains of a tile column sit
+// once in each direction per sweep (0.25 B per replica-site update), moved by
+// TMA bulk copies (cp.async.bulk; one or two contiguous 16-byte-aligned runs per tile
+// column, completing on the warp's own mbarrier).  Because all domains of a tile column sit
 // in one warp, sub-steps need __syncwarp() only - no block barrier anywhere in
 // the sweep.
 //
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 7 ? 2 : 1) sweep_warp_kernel(
     uint64_t *g = P.lat + (size_t)wl * L;             // column wl, contiguous in the site index
     const uint32_t stride = (Ts + 3u) & ~1u;          // words per warp buffer (even, >= Ts + 2)
     uint64_t *buf = smem + (size_t)warp * stride;
-    const bool vec = ((L | Ts) & 1u) == 0;            // 128-bit path needs even L and T_s
+    const bool vec = ((L | Ts) & 1u) == 0;            // 16-byte-aligned (TMA / 128-bit) path needs even L and T_s
     const uint32_t conn = P.connected;                // 1: connected multispin lattice (C10)
     const uint32_t odd = vec ? (start & 1u) : 0u;
     uint64_t *tile = buf + odd;                       // tile[y], y in [0, Ts)
