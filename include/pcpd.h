@@ -214,7 +214,8 @@ PCPD_API int pcpd_step_from_host(pcpd_t *h, const uint64_t *in_words, uint64_t n
  * the device keeps; e.g. a checkpoint written from the device layout): a chunk of columns is then one contiguous copy
  * straight into the lattice, with no staging buffer and no transpose, at the full host-to-device rate (the strided
  * copy of pcpd_step_from_host out of 8 W-byte rows runs at about half of it), and the call allocates nothing on the
- * device.  Chunks are as small as still fill the GPU.  Same result as pcpd_step_from_host on the transposed buffer, bit
+ * device.  Chunks are whole multiples of the most columns that fit two waves of warps, a short first one (the only
+ * exposed copy) and growing ones after it (PCPD_STEP_CHUNK = columns per chunk overrides: uniform chunks).  Same result as pcpd_step_from_host on the transposed buffer, bit
  * for bit.  in_columns: L*W uint64, pinned host memory for the copies to be asynchronous.  Synchronises. */
 PCPD_API int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t n_sweeps, uint32_t *out_counts);
 

@@ -680,8 +680,9 @@ int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t 
     if (!h || !in_columns) return fail(PCPD_ERR_ARG, "null argument");
     if (h->sweep + n_sweeps > 0xffffffffull) return fail(PCPD_ERR_RANGE, "sweep counter would exceed 2^32-1");
     const uint32_t L = (uint32_t)h->L, W = (uint32_t)h->W;
-    // chunk: as few columns as still give a launch two full waves of warps (2 x 148 SMs x 14 warps), so that the first,
-    // exposed copy is short; handles too small for two such chunks copy the whole lattice first
+    // chunk unit: the most columns that still fit two full waves of warps (2 x 148 SMs x 14 warps) - a launch of 2.2
+    // waves costs three wave-times, one of 1.98 two - so that the first, exposed copy is short and no launch ends in a
+    // nearly empty wave; handles too small for two such chunks copy the whole lattice first
     uint32_t cw = W;
     if (const char *e = getenv("PCPD_STEP_CHUNK")) {   // tuning hook: columns per chunk (0 = no pipelining)
         const long v = atol(e);
@@ -689,12 +690,37 @@ int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t 
     } else if (!h->thr && !h->force_block) {
         const uint64_t per_col = h->L / h->Ts;
         if (per_col > 0) {
-            const uint64_t want = (2ull * 148 * 14 + per_col - 1) / per_col;
-            if (want < W) cw = (uint32_t)want;
+            uint64_t unit = (2ull * 148 * 14) / per_col;
+            if (unit == 0) unit = 1;
+            if (2 * unit <= W) cw = (uint32_t)unit;
         }
     }
     if (h->thr || h->force_block) cw = W;
-    const uint32_t nchunks = (W + cw - 1) / cw;
+    // chunk boundaries: a short first chunk (its copy is the only exposed one), then chunks that grow by the factor by
+    // which copying a column is faster than sweeping it n_sweeps times, so that chunk c+1 has arrived when chunk c is
+    // done while the later, larger launches lose less to launch and tail overhead; at most four times the first.  The
+    // factor is an estimate from the measured configs (a sweep of a column costs about 0.0164 of its copy per Philox
+    // block executed per attempt: cfg4 ~12 blocks, ten sweeps: 2.0; cfg3 ~6.4 blocks: 1.05), clamped to [1, 2].
+    // PCPD_STEP_CHUNK: uniform chunks.
+    uint32_t bounds[66];
+    uint32_t nchunks = 0;
+    bounds[0] = 0;
+    {
+        const uint32_t nbd = (h->P.thd.nplanes + 1u) >> 1, nbp = (h->P.thp.nplanes + 1u) >> 1;
+        const double blocks = 1.0 + (nbd >= 5 ? 6.5 : nbd ? 1.0 : 0.0) + (h->P.pmask_paper ? 1.0 : nbp >= 5 ? 4.7 : nbp ? 1.0 : 0.0);
+        double grow = 0.0164 * blocks * (double)n_sweeps;
+        grow = grow < 1.0 ? 1.0 : grow > 2.0 ? 2.0 : grow;
+        if (getenv("PCPD_STEP_CHUNK")) grow = 1.0;
+        uint32_t w0 = 0;
+        double mult = 1.0;   // chunk size in units of cw: whole multiples, so that every launch stays wave-aligned
+        while (w0 < W && nchunks < 64) {
+            const uint32_t sz = cw * (uint32_t)(mult + 0.5);
+            const uint32_t nw = (W - w0 < sz + cw || nchunks == 63) ? W - w0 : sz;   // (a last chunk below one unit is merged)
+            w0 += nw;
+            bounds[++nchunks] = w0;
+            if (mult * grow <= 4.0) mult *= grow;
+        }
+    }
     int rc = ensure_copy_resources(h, nchunks);
     if (rc != PCPD_OK) return rc;
     cudaStream_t copy = h->copy_stream;
@@ -703,12 +729,12 @@ int pcpd_step_from_host_columns(pcpd_t *h, const uint64_t *in_columns, uint64_t 
     cudaError_t e = cudaEventRecord(h->copy_start, h->stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, h->copy_start, 0);
     for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
-        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        const uint32_t w0 = bounds[c], nw = bounds[c + 1] - w0;
         e = cudaMemcpyAsync(h->lat + (size_t)w0 * L, in_columns + (size_t)w0 * L, (size_t)nw * L * 8, cudaMemcpyHostToDevice, copy);
         if (e == cudaSuccess) e = cudaEventRecord(ev[c], copy);
     }
     for (uint32_t c = 0; e == cudaSuccess && c < nchunks; ++c) {
-        const uint32_t w0 = c * cw, nw = (w0 + cw <= W ? cw : W - w0);
+        const uint32_t w0 = bounds[c], nw = bounds[c + 1] - w0;
         e = cudaStreamWaitEvent(h->stream, ev[c], 0);
         if (e != cudaSuccess) break;
         SweepParams Pc = h->P;   // the chunk as a lattice of its own: columns w0 .. w0+nw-1 (columns never interact)
